@@ -1,0 +1,209 @@
+"""Pins for the oracle (no GPU): closed forms, brute force, invariants -- nothing here re-calls the
+oracle's own formula as the expected value.  Citations: P:L<n> = /root/reference/PAPER.md line."""
+import math, os
+import numpy as np
+import pytest
+from conftest import rel_l2
+from oracle import direct, analytic, nufft, prior, mbir
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _load(name):
+    return np.loadtxt(os.path.join(GOLD, name), comments="#")
+
+
+# ---------------------------------------------------------------- (D1) scale, sign, axes, centre
+def test_d1_golden_delta_row():
+    f = np.zeros((8, 8)); f[5, 2] = 1.0
+    row = direct.radon_direct(f, [math.pi / 5], 8, 4.0)[0]
+    assert np.allclose(row, _load("dirichlet_delta_n8.txt"), atol=1e-12)
+
+
+@pytest.mark.parametrize("s,tol", [(3.0, 1e-12), (2.0, 1e-7)])
+def test_d1_gaussian_closed_form(s, tol):
+    # eq. (2) P:L48 in closed form for a Gaussian blob; off-centre blob, non-integer centre:
+    # pins the scale (1/Nd, unit pixels), the sign of t, the x/y axes and the centre convention.
+    N, x0, y0, centre = 64, 5.0, -7.0, 33.75
+    x = np.arange(N) - N // 2
+    f = np.exp(-((x[None, :] - x0) ** 2 + (x[:, None] - y0) ** 2) / (2 * s * s))
+    ang = np.array([0.0, 0.3, math.pi / 2, 2.0, 3.0])
+    got = direct.radon_direct(f, ang, N, centre)
+    want = analytic.gaussian_projection(x0, y0, s, ang, N, centre)
+    assert rel_l2(got, want) < tol
+
+
+@pytest.mark.parametrize("centre", [4.0, 4.5, 3.25])
+def test_d1_equals_dirichlet_form(centre):
+    rng = np.random.default_rng(1)
+    f = rng.standard_normal((8, 8)); ang = rng.uniform(0, math.pi, 5)
+    assert rel_l2(direct.radon_direct(f, ang, 8, centre), direct.radon_dirichlet(f, ang, 8, centre)) < 1e-12
+
+
+def test_d1_axis_angles_reduce_to_fft_and_sums():
+    # theta = 0 integrates along y: column sums minus their Nyquist component; theta = pi/2: row sums.
+    rng = np.random.default_rng(2); N = 16
+    f = rng.standard_normal((N, N))
+    p = direct.radon_direct(f, [0.0, math.pi / 2], N, N / 2)
+    for row, cs in ((p[0], f.sum(axis=0)), (p[1], f.sum(axis=1))):
+        sgn = (-1.0) ** np.arange(N)
+        assert np.allclose(row, cs - sgn * np.sum(sgn * cs) / N, atol=1e-12)
+    # slice theorem (eq. (3)) on the library FFT: F1[Af](m) = fft2(f shifted)[0][m] at theta = 0
+    F1 = np.fft.fft(np.roll(p[0], -N // 2))                      # origin of t at bin N/2
+    F2 = np.fft.fft2(np.roll(f, (-N // 2, -N // 2), axis=(0, 1)))
+    m = np.arange(1, N // 2)
+    assert np.allclose(F1[m], F2[0, m], atol=1e-10) and np.allclose(F1[-m], F2[0, -m], atol=1e-10)
+    assert abs(F1[N // 2]) < 1e-10                               # Nyquist excluded (reading G2)
+
+
+def test_d2_is_transpose_bruteforce_and_identity():
+    rng = np.random.default_rng(3); N = 8
+    ang = rng.uniform(0, math.pi, 6); centre = 4.25
+    A = direct.dense_matrix(N, ang, N, centre)                   # Dirichlet form, independent code path
+    y = rng.standard_normal((6, N))
+    assert rel_l2(direct.backproject_direct(y, ang, N, centre).ravel(), A.T @ y.ravel()) < 1e-12
+    x = rng.standard_normal((N, N))
+    assert rel_l2(direct.radon_direct(x, ang, N, centre).ravel(), A @ x.ravel()) < 1e-12
+    N = 32; ang = rng.uniform(0, math.pi, 11)
+    x = rng.standard_normal((2, N, N)); y = rng.standard_normal((2, 11, N))
+    lhs = np.sum(direct.radon_direct(x, ang, N, 17.5) * y); rhs = np.sum(x * direct.backproject_direct(y, ang, N, 17.5))
+    assert abs(lhs - rhs) <= 1e-12 * abs(lhs)
+
+
+# ---------------------------------------------------------------- continuous line integral (loose by nature)
+def test_ellipse_analytic_and_ray_driven():
+    errs = []
+    for N in (64, 128):
+        x = np.arange(N) - N // 2
+        X, Y = np.meshgrid(x, x)
+        ell = [(0.1 * N, -0.05 * N, 0.3 * N, 0.2 * N, 0.4, 1.0), (-0.15 * N, 0.1 * N, 0.1 * N, 0.15 * N, 1.1, 0.5)]
+        ang = np.arange(12) * math.pi / 12
+        f = np.zeros((N, N)); want = np.zeros((12, N))
+        for (x0, y0, a, b, phi, rho) in ell:
+            c, s = math.cos(phi), math.sin(phi)
+            f += rho * ((((X - x0) * c + (Y - y0) * s) / a) ** 2 + ((-(X - x0) * s + (Y - y0) * c) / b) ** 2 <= 1)
+            want += analytic.ellipse_projection(x0, y0, a, b, phi, rho, ang, N, N / 2)
+        errs.append(rel_l2(direct.radon_direct(f, ang, N, N / 2), want))
+        assert rel_l2(analytic.radon_ray(f, ang, N, N / 2), want) < 0.03
+    assert errs[0] < 0.03 and errs[1] < 0.015 and errs[1] < errs[0]
+
+
+def test_ray_driven_gaussian():
+    N, s = 64, 6.0      # bilinear interpolation widens the blob by ~1/6 px^2: loose pin
+    x = np.arange(N) - N // 2
+    f = np.exp(-((x[None, :] - 4) ** 2 + (x[:, None] + 6) ** 2) / (2 * s * s))
+    ang = np.array([0.2, 1.3, 2.9])
+    assert rel_l2(analytic.radon_ray(f, ang, N, 31.5), analytic.gaussian_projection(4, -6, s, ang, N, 31.5)) < 5e-3
+
+
+# ---------------------------------------------------------------- the NUFFT approximation (eqs. (6)-(8))
+@pytest.mark.parametrize("centre", [32.0, 35.5])
+def test_nufft_within_error_bound_of_direct(centre):
+    # w ~ log10(1/eps) P:L87: W = 6 => eps ~ 1e-6..1e-5
+    rng = np.random.default_rng(4); N = 64
+    ang = np.arange(45) * math.pi / 45
+    f = rng.random((N, N)); y = rng.standard_normal((45, N))
+    assert rel_l2(nufft.radon_nufft(f, ang, N, centre), direct.radon_direct(f, ang, N, centre)) < 2e-5
+    assert rel_l2(nufft.backproject_nufft(y, ang, N, centre), direct.backproject_direct(y, ang, N, centre)) < 2e-5
+
+
+def test_nufft_vs_bruteforce_matrix_8x8_and_exact_transpose():
+    rng = np.random.default_rng(5); N = 8
+    ang = rng.uniform(0, math.pi, 7); centre = 3.75
+    A = direct.dense_matrix(N, ang, N, centre)
+    An = np.stack([nufft.radon_nufft(e.reshape(N, N), ang, N, centre).ravel() for e in np.eye(N * N)], axis=1)
+    Bn = np.stack([nufft.backproject_nufft(e.reshape(7, N), ang, N, centre).ravel() for e in np.eye(7 * N)], axis=1)
+    assert np.abs(An - A).max() < 3e-5 * np.abs(A).max()
+    assert np.abs(Bn - An.T).max() < 1e-13 * np.abs(An).max()    # exact transpose, not just approximate
+
+
+def test_nufft_adjoint_identity_and_stage_transposes():
+    rng = np.random.default_rng(6); N, na = 32, 9; G = 64
+    ang = rng.uniform(0, math.pi, na)
+    x = rng.standard_normal((N, N)); y = rng.standard_normal((na, N))
+    lhs = np.sum(nufft.radon_nufft(x, ang, N, 15.5) * y); rhs = np.sum(x * nufft.backproject_nufft(y, ang, N, 15.5))
+    assert abs(lhs - rhs) <= 1e-12 * abs(lhs)
+    Gh = rng.standard_normal((G, G)) + 1j * rng.standard_normal((G, G))
+    c = rng.standard_normal((na, N - 1)) + 1j * rng.standard_normal((na, N - 1))
+    assert abs(np.vdot(c, nufft.gather(Gh, ang, N)) - np.vdot(nufft.spread(c, ang, N, G), Gh)) < 1e-10
+    p = rng.standard_normal((na, N))
+    assert abs(np.vdot(p, nufft.radial_inverse(c, N, 15.5)).real - np.vdot(nufft.radial_forward(p, N, 15.5), c).real) < 1e-10
+
+
+def test_kb_window_properties():
+    # phihat is the Fourier transform of phi: check by quadrature (independent of the closed form)
+    W, G = 6, 128
+    r = np.linspace(-3, 3, 200001)
+    phi = nufft.kb_window(r)
+    for xj in (0, 10, 31):
+        num = np.trapezoid(phi * np.cos(2 * np.pi * r * xj / G), r)
+        assert abs(num * nufft.kb_deapod(64, G)[xj + 32] - 1.0) < 1e-6
+    assert nufft.kb_window(3.0) > 0 and nufft.kb_window(3.0000001) == 0 and abs(nufft.kb_beta() - math.pi * math.sqrt(19.45)) < 1e-14
+
+
+# ---------------------------------------------------------------- prior, eqs. (12)-(13)
+P, SIG, C = 1.2, 1 / 0.7, 1e-4
+
+
+def test_prior_golden_spot_values():
+    for D, hv, dv in _load("qggmrf_spot.txt"):
+        assert abs(prior.h(D, P, SIG, C) - hv) < 1e-12 and abs(prior.dh(D, P, SIG, C) - dv) < 1e-12
+        assert abs(prior.dh(-D, P, SIG, C) + dv) < 1e-12
+    assert prior.dh(0.0, P, SIG, C) == 0.0
+
+
+def test_prior_weights_and_bruteforce_H():
+    offs = prior.offsets26()
+    assert len(offs) == 26 and abs(sum(prior.weight(o) for o in offs) - 1.0) < 1e-14
+    assert abs(prior.weight((0, 0, 1)) - 0.0523448) < 1e-7 and abs(prior.weight((1, 1, 1)) - 0.0302213) < 1e-7
+    rng = np.random.default_rng(7); f = rng.standard_normal((3, 4, 5))
+    tot = 0.0                                                    # plain loops over unordered pairs, eq. (12)
+    idx = [(z, y, x) for z in range(3) for y in range(4) for x in range(5)]
+    for a in idx:
+        for b in idx:
+            d = max(abs(a[k] - b[k]) for k in range(3))
+            if d == 1 and a < b:
+                dist = math.sqrt(sum((a[k] - b[k]) ** 2 for k in range(3)))
+                u = abs(f[a] - f[b]) / SIG
+                tot += (1 / dist / (6 + 12 / math.sqrt(2) + 8 / math.sqrt(3))) * u * u / (C + u ** (2 - P))
+    assert abs(prior.H(f, P, SIG, C) - tot) < 1e-12 * tot
+
+
+def test_prior_gradient_finite_difference():
+    rng = np.random.default_rng(8); f = rng.standard_normal((5, 6, 7))
+    g = prior.gradH(f, P, SIG, C)
+    eps = 1e-6
+    for pos in [(0, 0, 0), (2, 3, 3), (4, 5, 6), (1, 0, 6), (2, 2, 0)]:
+        fp = f.copy(); fm = f.copy(); fp[pos] += eps; fm[pos] -= eps
+        fd = (prior.H(fp, P, SIG, C) - prior.H(fm, P, SIG, C)) / (2 * eps)
+        assert abs(fd - g[pos]) < 1e-6 * max(1.0, abs(fd))
+    assert np.all(prior.gradH(np.full((3, 4, 5), 0.7), P, SIG, C) == 0.0)
+
+
+# ---------------------------------------------------------------- MBIR loop invariants (iterate sequence unpinned vs paper)
+def test_mbir_invariants():
+    rng = np.random.default_rng(9); N, na = 16, 12
+    ang = np.arange(na) * math.pi / na
+    truth = np.zeros((2, N, N)); truth[:, 5:11, 4:9] = 1.0; truth[1, 7:9, 6:12] += 0.5
+    b = nufft.radon_nufft(truth, ang, N, 8.0) + 0.01 * rng.standard_normal((2, na, N))
+    L, lam_hat = mbir.lipschitz(N, ang, N, 8.0, P, SIG, C, 1.0)
+    assert 0.5 * na * N < lam_hat < 2.0 * na * N
+    x1, log1 = mbir.mbir(b, ang, N, 8.0, P, SIG, C, 1.0, L, 1)
+    assert rel_l2(x1, nufft.backproject_nufft(b, ang, N, 8.0) / L) < 1e-12      # first iterate = A^T b / L
+    x, log = mbir.mbir(b, ang, N, 8.0, P, SIG, C, 1.0, L, 25)
+    F = [0.5 * np.sum(b * b)] + [l["F"] for l in log]
+    assert all(F[i + 1] <= F[i] for i in range(len(F) - 1)) and F[-1] < 0.5 * F[0]
+
+
+def test_mbir_lambda0_converges_to_least_squares():
+    N, na = 8, 10
+    ang = np.arange(na) * math.pi / na
+    rng = np.random.default_rng(10)
+    b = rng.standard_normal((1, na, N))
+    An = np.stack([nufft.radon_nufft(e.reshape(N, N), ang, N, 4.0).ravel() for e in np.eye(N * N)], axis=1)
+    xs, res, *_ = np.linalg.lstsq(An, b.ravel(), rcond=None)
+    Fstar = 0.5 * np.sum((An @ xs - b.ravel()) ** 2)
+    Lc = 1.02 * np.linalg.norm(An, 2) ** 2
+    x, log = mbir.mbir(b, ang, N, 4.0, P, SIG, C, 0.0, Lc, 400)
+    assert log[-1]["F"] - Fstar < 1e-6 * Fstar + 1e-9
+    assert np.linalg.norm(An.T @ (An @ x.ravel() - b.ravel())) < 1e-3 * np.linalg.norm(An.T @ b.ravel())
