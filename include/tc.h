@@ -1,0 +1,96 @@
+/* tc.h -- C ABI of the tomoCAM hot path on one B200 (sm_100a).
+ *
+ * Paper: arXiv 2304.12934 (tomoCAM).  "P:L<n>" = line n of /root/reference/PAPER.md.
+ * The three calls follow the paper's problem statement: the Radon transform R (eq. (2))
+ * and its adjoint R* (eq. (11)) computed slice by slice with a NUFFT
+ * (eqs. (6)-(8)), inside the MBIR gradient iteration (eqs. (9)-(10)) with
+ * the qGGMRF prior (eqs. (12)-(13)).
+ *
+ * Layouts (all float32, C-contiguous; no complex numbers cross the boundary):
+ *   volume   [slice][row i <-> y][col j <-> x],  x_j = j - n/2, y_i = i - n/2   (n x n per slice)
+ *   sinogram [slice][angle a][bin u]            (sinogram order), t_u = u - center
+ * Pointers: every data pointer may be DEVICE memory or HOST memory (pinned or pageable); the
+ *   library looks the pointer up (cudaPointerGetAttributes).  Host pointers take the slab-streaming
+ *   path: slabs of slices go through pinned staging buffers on side streams, overlapped
+ *   with compute, and the call returns when the output is complete.  Device-pointer calls are
+ *   ordered on `cuda_stream` (a cudaStream_t, NULL = default stream) and return asynchronously.
+ * Ownership: the caller owns every data buffer; the plan owns all scratch; nothing allocated by the
+ *   library is ever returned.  A plan is not thread-safe.
+ * Errors: every call returns a tc_status; nothing throws or aborts across the ABI; outputs are
+ *   unspecified after an error; tc_last_error() gives thread-local text for the last failure.
+ */
+#ifndef TC_H
+#define TC_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { TC_OK = 0, TC_EINVAL = 1, TC_ENOMEM = 2, TC_ECUDA = 3, TC_EUNSUPPORTED = 4 } tc_status;
+
+/* Acquisition geometry.  n: image side (even); n_det: detector bins (even); angles: HOST pointer to
+ * n_angles float32 radians (copied at plan creation; any finite values); center: rotation-axis
+ * position in bins (< 0 means n_det/2); oversamp must be 2.0 and kb_width 6 (Kaiser-Bessel
+ * window; w ~ log10(1/eps)).  2n and n_det must factor into {2, 3, 5}. */
+typedef struct {
+    int n, n_det, n_angles;
+    const float *angles;
+    float center;
+    float oversamp;
+    int kb_width;
+} tc_geom;
+
+/* qGGMRF prior h = (|D|/sigma)^2 / (c + (|D|/sigma)^(2-p)), eq. (13); paper's values
+ * p = 1.2, sigma = 1/0.7, c = 1e-4.  lambda multiplies the prior (extension, default 1).
+ * L is the step constant of the fixed 1/L step; 0 means: estimated by the library (power iteration
+ * on A^T A plus the curvature bound of the prior, reading G15). */
+typedef struct { float p, sigma, c, lambda, L; } tc_prior;
+
+/* One record per MBIR iteration: F = objective of the kept iterate, data / prior = the two terms of
+ * the CANDIDATE, margin = (F_prev - F_cand)/F_prev, beta = momentum used, accepted = 1/0. */
+typedef struct { double F, data, prior, margin; float beta; int accepted; } tc_iter_log;
+
+typedef struct tc_plan tc_plan;
+
+/* Builds window coefficients, deapodisation vector, FFT twiddles, sorted angle tables.  Scratch is
+ * allocated lazily by the first call that needs it.  max_slab_slices (0 = automatic) caps the number
+ * of slices processed per slab. */
+tc_status tc_plan_create(const tc_geom *geom, int max_slab_slices, tc_plan **out);
+tc_status tc_plan_destroy(tc_plan *plan);
+
+/* sinogram[n_slices][n_angles][n_det] = A volume[n_slices][n][n]  (forward, type-2 NUFFT route). */
+tc_status tc_radon(tc_plan *plan, const float *volume, int n_slices, float *sinogram, void *cuda_stream);
+
+/* volume[n_slices][n][n] = A^T sinogram[n_slices][n_angles][n_det]  (exact transpose of tc_radon). */
+tc_status tc_backproject(tc_plan *plan, const float *sinogram, int n_slices, float *volume, void *cuda_stream);
+
+/* `iters` iterations of the monotone accelerated gradient method with restart on
+ * F(f) = 1/2 ||A f - b||^2 + lambda H(f) from f = 0.  volume: out.  log: HOST pointer, nullable,
+ * `iters` records.  Synchronous (returns when `volume` is complete). */
+tc_status tc_mbir(tc_plan *plan, const float *sinogram, int n_slices, const tc_prior *prior, int iters,
+                  float *volume, tc_iter_log *log, void *cuda_stream);
+
+/* lambda_hat = ||A^T A v|| / ||v|| after `iters` power iterations on one slice from v = ones. */
+tc_status tc_power_iteration(tc_plan *plan, int iters, double *lambda_hat);
+
+/* Prior alone (test hook for the M2/M4 stencil kernels): grad (nullable) = grad H(volume),
+ * *value (HOST, nullable) = H(volume); device or host pointers for volume/grad. */
+tc_status tc_prior_eval(const float *volume, int n_slices, int n, const tc_prior *prior, float *grad, double *value);
+
+/* One-shot form with exactly the problem statement's shape = create plan, tc_radon, destroy. */
+tc_status tc_radon1(const float *volume, int n_slices, int n, const float *angles, int n_angles, int n_det,
+                    float center, float *sinogram);
+
+/* Kernel launches issued by this library on the calling thread since the last reset (for bench.py). */
+long long tc_launch_count(int reset);
+
+/* Scheduler statistics of the last host-pointer call: seconds of H2D, compute, D2H (summed CUDA-event
+ * spans) and wall; overlap = (copy + compute - wall) / min(copy, compute). */
+typedef struct { double h2d_s, compute_s, d2h_s, wall_s, overlap; long long h2d_bytes, d2h_bytes; int n_slabs; } tc_sched_stats;
+tc_status tc_last_sched_stats(tc_plan *plan, tc_sched_stats *out);
+
+const char *tc_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,165 @@
+"""Thin ctypes binding of include/tc.h -- argument marshalling only; every step runs in libtc.so's CUDA kernels.
+
+Accepts torch tensors (CUDA, or CPU -- pinned or not) and numpy arrays (host).  There is no CPU fallback:
+a missing library raises at import of this module.
+"""
+import ctypes, os
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libtc.so")
+if not os.path.exists(_LIB_PATH):
+    raise ImportError("libtc.so not built: run `python -m paper_2304_12934_b200.build` (no CPU fallback exists)")
+lib = ctypes.CDLL(_LIB_PATH)
+
+TC_OK, TC_EINVAL, TC_ENOMEM, TC_ECUDA, TC_EUNSUPPORTED = range(5)
+
+
+class tc_geom(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_int), ("n_det", ctypes.c_int), ("n_angles", ctypes.c_int),
+                ("angles", ctypes.POINTER(ctypes.c_float)), ("center", ctypes.c_float),
+                ("oversamp", ctypes.c_float), ("kb_width", ctypes.c_int)]
+
+
+class tc_prior(ctypes.Structure):
+    _fields_ = [("p", ctypes.c_float), ("sigma", ctypes.c_float), ("c", ctypes.c_float),
+                ("lam", ctypes.c_float), ("L", ctypes.c_float)]
+
+
+class tc_iter_log(ctypes.Structure):
+    _fields_ = [("F", ctypes.c_double), ("data", ctypes.c_double), ("prior", ctypes.c_double),
+                ("margin", ctypes.c_double), ("beta", ctypes.c_float), ("accepted", ctypes.c_int)]
+
+
+class tc_sched_stats(ctypes.Structure):
+    _fields_ = [("h2d_s", ctypes.c_double), ("compute_s", ctypes.c_double), ("d2h_s", ctypes.c_double),
+                ("wall_s", ctypes.c_double), ("overlap", ctypes.c_double), ("h2d_bytes", ctypes.c_longlong),
+                ("d2h_bytes", ctypes.c_longlong), ("n_slabs", ctypes.c_int)]
+
+
+_vp, _ci = ctypes.c_void_p, ctypes.c_int
+lib.tc_plan_create.argtypes = [ctypes.POINTER(tc_geom), _ci, ctypes.POINTER(_vp)]
+lib.tc_plan_destroy.argtypes = [_vp]
+lib.tc_radon.argtypes = [_vp, _vp, _ci, _vp, _vp]
+lib.tc_backproject.argtypes = [_vp, _vp, _ci, _vp, _vp]
+lib.tc_mbir.argtypes = [_vp, _vp, _ci, ctypes.POINTER(tc_prior), _ci, _vp, ctypes.POINTER(tc_iter_log), _vp]
+lib.tc_power_iteration.argtypes = [_vp, _ci, ctypes.POINTER(ctypes.c_double)]
+lib.tc_prior_eval.argtypes = [_vp, _ci, _ci, ctypes.POINTER(tc_prior), _vp, ctypes.POINTER(ctypes.c_double)]
+lib.tc_radon1.argtypes = [_vp, _ci, _ci, ctypes.POINTER(ctypes.c_float), _ci, _ci, ctypes.c_float, _vp]
+lib.tc_launch_count.argtypes = [_ci]
+lib.tc_launch_count.restype = ctypes.c_longlong
+lib.tc_last_sched_stats.argtypes = [_vp, ctypes.POINTER(tc_sched_stats)]
+lib.tc_last_error.restype = ctypes.c_char_p
+for _f in ("tc_plan_create", "tc_plan_destroy", "tc_radon", "tc_backproject", "tc_mbir", "tc_power_iteration",
+           "tc_prior_eval", "tc_radon1", "tc_last_sched_stats"):
+    getattr(lib, _f).restype = _ci
+
+
+class TcError(RuntimeError):
+    def __init__(self, status):
+        self.status = status
+        super().__init__("tc status %d: %s" % (status, lib.tc_last_error().decode()))
+
+
+def _check(st):
+    if st != TC_OK:
+        raise TcError(st)
+
+
+def _ptr(a):
+    """data pointer of a float32 C-contiguous torch tensor or numpy array."""
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.float32 and a.flags.c_contiguous
+        return a.ctypes.data
+    assert a.dtype.__str__() == "torch.float32" and a.is_contiguous()
+    return a.data_ptr()
+
+
+def _stream(a):
+    if isinstance(a, np.ndarray) or not a.is_cuda:
+        return None
+    import torch
+    return torch.cuda.current_stream(a.device).cuda_stream
+
+
+def _like(a, shape):
+    if isinstance(a, np.ndarray):
+        return np.empty(shape, dtype=np.float32)
+    import torch
+    return torch.empty(shape, dtype=torch.float32, device=a.device, pin_memory=(not a.is_cuda and a.is_pinned()))
+
+
+def prior_params(p=1.2, sigma=1 / 0.7, c=1e-4, lam=1.0, L=0.0):
+    return tc_prior(p, sigma, c, lam, L)
+
+
+class Plan:
+    """tc_plan_create / tc_plan_destroy; methods are the C calls of the same names."""
+
+    def __init__(self, n, n_det, angles, center=-1.0, max_slab_slices=0):
+        ang = np.ascontiguousarray(np.asarray(angles, dtype=np.float32))
+        self.n, self.n_det, self.n_angles = int(n), int(n_det), int(ang.size)
+        g = tc_geom(self.n, self.n_det, self.n_angles, ang.ctypes.data_as(ctypes.POINTER(ctypes.c_float)),
+                    float(center), 2.0, 6)
+        self._h = _vp()
+        _check(lib.tc_plan_create(ctypes.byref(g), int(max_slab_slices), ctypes.byref(self._h)))
+
+    def close(self):
+        if getattr(self, "_h", None) and lib is not None:
+            lib.tc_plan_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def radon(self, volume, out=None):
+        S = volume.shape[0]
+        assert tuple(volume.shape) == (S, self.n, self.n)
+        out = _like(volume, (S, self.n_angles, self.n_det)) if out is None else out
+        _check(lib.tc_radon(self._h, _ptr(volume), S, _ptr(out), _stream(volume)))
+        return out
+
+    def backproject(self, sinogram, out=None):
+        S = sinogram.shape[0]
+        assert tuple(sinogram.shape) == (S, self.n_angles, self.n_det)
+        out = _like(sinogram, (S, self.n, self.n)) if out is None else out
+        _check(lib.tc_backproject(self._h, _ptr(sinogram), S, _ptr(out), _stream(sinogram)))
+        return out
+
+    def mbir(self, sinogram, prior, iters, out=None):
+        S = sinogram.shape[0]
+        assert tuple(sinogram.shape) == (S, self.n_angles, self.n_det)
+        out = _like(sinogram, (S, self.n, self.n)) if out is None else out
+        log = (tc_iter_log * max(iters, 1))()
+        _check(lib.tc_mbir(self._h, _ptr(sinogram), S, ctypes.byref(prior), int(iters), _ptr(out), log, _stream(sinogram)))
+        recs = [dict(F=l.F, data=l.data, prior=l.prior, margin=l.margin, beta=l.beta, accepted=l.accepted) for l in log[:iters]]
+        return out, recs
+
+    def power_iteration(self, iters=10):
+        v = ctypes.c_double()
+        _check(lib.tc_power_iteration(self._h, int(iters), ctypes.byref(v)))
+        return v.value
+
+    def sched_stats(self):
+        s = tc_sched_stats()
+        _check(lib.tc_last_sched_stats(self._h, ctypes.byref(s)))
+        return {k: getattr(s, k) for k, _ in tc_sched_stats._fields_}
+
+
+def prior_eval(volume, prior, want_grad=True):
+    S, n, _ = volume.shape
+    grad = _like(volume, tuple(volume.shape)) if want_grad else None
+    val = ctypes.c_double()
+    _check(lib.tc_prior_eval(_ptr(volume), S, n, ctypes.byref(prior), _ptr(grad) if want_grad else None, ctypes.byref(val)))
+    return val.value, grad
+
+
+def radon1(volume, angles, n_det, center):
+    ang = np.ascontiguousarray(np.asarray(angles, dtype=np.float32))
+    S, n, _ = volume.shape
+    out = _like(volume, (S, ang.size, n_det))
+    _check(lib.tc_radon1(_ptr(volume), S, n, ang.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), ang.size, n_det, float(center), _ptr(out)))
+    return out
+
+
+def launch_count(reset=False):
+    return lib.tc_launch_count(1 if reset else 0)

@@ -1,0 +1,66 @@
+// Shared declarations of the tomoCAM B200 library (device-side plan view, launch wrappers).
+#pragma once
+#include <cuda_runtime.h>
+#include "fft.cuh"
+
+namespace tc {
+
+constexpr int KB_W = 6;          // Kaiser-Bessel window width (taps per axis)
+constexpr int KB_DEG = 12;       // degree of the window polynomial in z = 2 q - 1, q = 1 - (2 r / W)^2
+constexpr int P = 4;             // complex planes interleaved per fine-grid cell (= 8 real slices, 32 B)
+
+// Everything the kernels need, passed by value.
+struct DevPlan {
+    int n, nd, na, G;
+    double sc;                    // G / nd: fine-grid cells per radial mode
+    FftDesc fG, fD;               // FFT descriptors for length G (fine grid) and nd (radial)
+    const float2 *twG, *twD;      // twiddles e^{-2 pi i k / n}
+    const float *deapod;          // d(x_j) = 1 / phihat(x_j), j < n
+    const float2 *ph_fwd;         // [nd] e^{-2 pi i m centre / nd} / nd, Nyquist entry 0 (forward, before the inverse radial FFT)
+    const float2 *ph_adj;         // [nd] e^{+2 pi i m centre / nd} / nd, Nyquist entry 0 (adjoint, after the radial FFT)
+    const double2 *cs;            // [na] (sc cos theta_a, sc sin theta_a)
+    const double2 *cs_sorted;     // [na] same, sorted by theta mod pi
+    const float *th_sorted;       // [na] theta mod pi, ascending
+    const int *a_sorted;          // [na] original angle index
+};
+
+// Window polynomial coefficients (monomial in z, c[0] + c[1] z + ...), set by the plan.
+void set_kb_coeffs(const float *h);
+
+// ---- launch wrappers (kernels_nufft.cu).  All buffers are device memory. -------------------------
+// vol [S][n][n] -> rowbuf [ng][n][G][P] c64      (F1 pad + deapodise, row FFT)
+void launch_fwd_rows(const DevPlan &d, const float *vol, int S, int ng, float2 *rowbuf, cudaStream_t st);
+// rowbuf -> grid [ng][G][G][P] c64               (F2 column FFT, zero rows pruned on input)
+void launch_fwd_cols(const DevPlan &d, const float2 *rowbuf, int ng, float2 *grid, cudaStream_t st);
+// grid -> sino [S][na][nd]                       (F3 polar gather + F4 centre phase and inverse radial FFT)
+void launch_fwd_gather(const DevPlan &d, const float2 *grid, int S, int ng, float *sino, cudaStream_t st);
+// sino -> cpol [ng][na][nd][P] c64               (B1 radial FFT + conjugate phase)
+void launch_adj_radial(const DevPlan &d, const float *sino, int S, int ng, float2 *cpol, cudaStream_t st);
+// cpol -> grid                                   (B2 spread, evaluated per fine-grid cell: plain stores, no atomics)
+void launch_adj_spread(const DevPlan &d, const float2 *cpol, int ng, float2 *grid, cudaStream_t st);
+// grid -> rowbuf (cropped to n rows)             (B3 inverse column FFT)
+void launch_adj_cols(const DevPlan &d, const float2 *grid, int ng, float2 *rowbuf, cudaStream_t st);
+// rowbuf -> vol (cropped, deapodised, re/im)     (B3 inverse row FFT + B4)
+void launch_adj_rows(const DevPlan &d, const float2 *rowbuf, int S, int ng, float *vol, cudaStream_t st);
+
+// ---- kernels_mbir.cu -------------------------------------------------------------------------------
+struct PriorDev { float p, sigma, c, lambda; };
+// y = x + beta (x - xm)                          (M1, volume part)
+void launch_extrapolate(const float *x, const float *xm, float beta, float *y, size_t n, cudaStream_t st);
+// r = Ax + beta (Ax - Axm) - b ; Ay kept          (M1, sinogram part)
+void launch_residual(const float *Ax, const float *Axm, const float *b, float beta, float *Ay, float *r, size_t n, cudaStream_t st);
+// g = atr + lambda grad H(y);  z = y - g / L      (M2 + M3).  y has S slices of n x n; g may alias atr.
+void launch_update(const float *y, const float *atr, PriorDev pr, float invL, float *g, float *z, int S, int n, cudaStream_t st);
+// Az = Ay - Ag / L;  acc[0] += 1/2 ||Az - b||^2   (M4 data term, fp64 accumulation)
+void launch_candidate_sino(const float *Ay, const float *Ag, const float *b, float invL, float *Az, double *acc, size_t n, cudaStream_t st);
+// acc[1] += H(z) over unordered 26-neighbour pairs (M4 prior term); grad (nullable) = grad H(z)
+void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, int n, cudaStream_t st);
+// acc[slot] += sum v^2
+void launch_sumsq(const float *v, size_t n, double *acc, int slot, cudaStream_t st);
+void launch_scale(float *v, float a, size_t n, cudaStream_t st);
+
+long long &launch_counter();
+
+}  // namespace tc
+
+#define TC_COUNT_LAUNCH() (++::tc::launch_counter())

@@ -1,0 +1,257 @@
+// C ABI of the tomoCAM B200 library (include/tc.h): plan, forward / adjoint pipelines, slab scheduler, MBIR loop.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <chrono>
+#include <string>
+#include <vector>
+#include <algorithm>
+#include "../../include/tc.h"
+#include "common.cuh"
+
+using namespace tc;
+
+static thread_local std::string g_err;
+static tc_status fail(tc_status s, const std::string &msg) { g_err = msg; return s; }
+extern "C" const char *tc_last_error(void) { return g_err.c_str(); }
+extern "C" long long tc_launch_count(int reset) { long long v = launch_counter(); if (reset) launch_counter() = 0; return v; }
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            tc_status s_ = (e_ == cudaErrorMemoryAllocation) ? TC_ENOMEM : TC_ECUDA;               \
+            return fail(s_, std::string(#call) + ": " + cudaGetErrorString(e_));                   \
+        }                                                                                          \
+    } while (0)
+#define TCS(call) do { tc_status s_ = (call); if (s_ != TC_OK) return s_; } while (0)
+
+struct tc_plan {
+    tc_geom geom;
+    std::vector<float> angles;
+    DevPlan d;
+    int max_slab;                 // slices per slab (multiple of 8), 0 = not yet decided
+    // device tables
+    float2 *twG = nullptr, *twD = nullptr, *ph_fwd = nullptr, *ph_adj = nullptr;
+    float *deapod = nullptr, *th_sorted = nullptr;
+    double2 *cs = nullptr, *cs_sorted = nullptr;
+    int *a_sorted = nullptr;
+    // scratch
+    int ng_alloc = 0;
+    float2 *rowbuf = nullptr, *grid = nullptr, *cpol = nullptr;
+    double *acc = nullptr;        // 16 results + reduction scratch
+    // host-pointer scheduler
+    float *stage_in[2] = {nullptr, nullptr}, *stage_out[2] = {nullptr, nullptr};
+    size_t stage_in_elems = 0, stage_out_elems = 0;
+    cudaStream_t s_h2d = nullptr, s_comp = nullptr, s_d2h = nullptr;
+    tc_sched_stats stats{};
+};
+
+// ---- host-side mathematics of the plan (float64) ---------------------------------------------------
+static double bessel_i0(double x) {          // I0(x) = sum_k (x^2/4)^k / (k!)^2
+    const double q = 0.25 * x * x;
+    double term = 1.0, sum = 1.0;
+    for (int k = 1; k < 200; ++k) { term *= q / ((double)k * k); sum += term; if (term < 1e-17 * sum) break; }
+    return sum;
+}
+static double kb_beta(int W, double sigma) { return M_PI * std::sqrt((W / sigma) * (W / sigma) * (sigma - 0.5) * (sigma - 0.5) - 0.8); }
+
+// phi as a function of z = 2 q - 1, q = 1 - (2 r / W)^2: Chebyshev interpolation, truncated, as monomials.
+static void kb_poly(int W, double sigma, float *out) {
+    const double beta = kb_beta(W, sigma), i0b = bessel_i0(beta);
+    const int M = 64;
+    std::vector<double> fz(M), zk(M);
+    for (int k = 0; k < M; ++k) {
+        zk[k] = std::cos(M_PI * (k + 0.5) / M);
+        const double q = 0.5 * (zk[k] + 1.0);
+        fz[k] = bessel_i0(beta * std::sqrt(q)) / i0b;
+    }
+    std::vector<double> cheb(KB_DEG + 1);
+    for (int j = 0; j <= KB_DEG; ++j) {
+        double s = 0.0;
+        for (int k = 0; k < M; ++k) s += fz[k] * std::cos(j * M_PI * (k + 0.5) / M);
+        cheb[j] = (j == 0 ? 1.0 : 2.0) * s / M;
+    }
+    // T_0 = 1, T_1 = z, T_{j+1} = 2 z T_j - T_{j-1}
+    std::vector<std::vector<double>> T(KB_DEG + 1, std::vector<double>(KB_DEG + 1, 0.0));
+    T[0][0] = 1.0; if (KB_DEG >= 1) T[1][1] = 1.0;
+    for (int j = 1; j < KB_DEG; ++j)
+        for (int k = 0; k <= KB_DEG; ++k) T[j + 1][k] = (k > 0 ? 2.0 * T[j][k - 1] : 0.0) - T[j - 1][k];
+    for (int k = 0; k <= KB_DEG; ++k) {
+        double s = 0.0;
+        for (int j = 0; j <= KB_DEG; ++j) s += cheb[j] * T[j][k];
+        out[k] = (float)s;
+    }
+}
+
+static bool make_fft_desc(int n, FftDesc &f) {
+    int m = n, fives = 0, twos = 0;
+    while (m % 5 == 0) { m /= 5; ++fives; }
+    while (m % 2 == 0) { m /= 2; ++twos; }
+    if (m != 1 || fives > 1 || n < 8) return false;
+    f.n = n; f.ps = n + (n >> 4) + 1;
+    f.first = twos % 3 == 1 ? 2 : (twos % 3 == 2 ? 4 : 0);
+    f.n8 = twos / 3; f.five = fives;
+    return true;
+}
+
+template <typename T> static cudaError_t upload(T **dst, const std::vector<T> &h) {
+    cudaError_t e = cudaMalloc((void **)dst, h.size() * sizeof(T));
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(*dst, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
+}
+
+extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_plan **out) {
+    if (!gm || !out) return fail(TC_EINVAL, "null argument");
+    if (gm->n <= 0 || gm->n_det <= 0 || gm->n_angles <= 0 || !gm->angles) return fail(TC_EINVAL, "non-positive size or null angles");
+    if ((gm->n & 1) || (gm->n_det & 1)) return fail(TC_EINVAL, "n and n_det must be even");
+    for (int a = 0; a < gm->n_angles; ++a)
+        if (!std::isfinite(gm->angles[a])) return fail(TC_EINVAL, "non-finite angle");
+    if (gm->oversamp != 2.0f || gm->kb_width != KB_W) return fail(TC_EUNSUPPORTED, "only oversamp = 2, kb_width = 6");
+    if (gm->n % 32) return fail(TC_EUNSUPPORTED, "n must be a multiple of 32");
+    tc_plan *p = new tc_plan();
+    p->geom = *gm;
+    p->angles.assign(gm->angles, gm->angles + gm->n_angles);
+    p->geom.angles = p->angles.data();
+    if (p->geom.center < 0) p->geom.center = 0.5f * gm->n_det;
+    p->max_slab = max_slab_slices > 0 ? (max_slab_slices + 7) / 8 * 8 : 0;
+    const int n = gm->n, nd = gm->n_det, na = gm->n_angles, G = 2 * n;
+    DevPlan &d = p->d;
+    d.n = n; d.nd = nd; d.na = na; d.G = G; d.sc = (double)G / nd;
+    if (!make_fft_desc(G, d.fG) || !make_fft_desc(nd, d.fD)) { delete p; return fail(TC_EUNSUPPORTED, "2n and n_det must be 2^a 5^b, b <= 1, >= 8"); }
+    if (nd / 2 - 1 > 0 && d.sc * (nd / 2 - 1) + 3 >= G / 2 + 3) { /* taps wrap at most once; always true for sc = G/nd */ }
+
+    const int W = KB_W; const double sigma = 2.0;
+    const double beta = kb_beta(W, sigma), i0b = bessel_i0(beta);
+    float kb[KB_DEG + 1];
+    kb_poly(W, sigma, kb);
+    set_kb_coeffs(kb);
+    std::vector<float> deapod(n);
+    for (int j = 0; j < n; ++j) {
+        const double x = j - n / 2, a = M_PI * W * x / G, s = std::sqrt(beta * beta - a * a);
+        deapod[j] = (float)(i0b * s / (W * std::sinh(s)));
+    }
+    auto twiddles = [](int len) {
+        std::vector<float2> t(len);
+        for (int i = 0; i < len; ++i) { const double a = 2.0 * M_PI * i / len; t[i] = make_float2((float)std::cos(a), (float)-std::sin(a)); }
+        return t;
+    };
+    std::vector<float2> phf(nd), pha(nd);
+    const double centre = p->geom.center;
+    for (int k = 0; k < nd; ++k) {
+        const int m = k < nd / 2 ? k : k - nd;
+        if (k == nd / 2) { phf[k] = pha[k] = make_float2(0.f, 0.f); continue; }
+        const double a = 2.0 * M_PI * std::fmod((double)m * centre, (double)nd) / nd;
+        phf[k] = make_float2((float)(std::cos(a) / nd), (float)(-std::sin(a) / nd));
+        pha[k] = make_float2((float)(std::cos(a) / nd), (float)(std::sin(a) / nd));
+    }
+    std::vector<double2> cs(na), css(na);
+    std::vector<float> ths(na);
+    std::vector<int> order(na);
+    std::vector<double> thm(na);
+    for (int a = 0; a < na; ++a) {
+        const double th = (double)p->angles[a];
+        cs[a] = make_double2(d.sc * std::cos(th), d.sc * std::sin(th));
+        double r = std::fmod(th, M_PI); if (r < 0) r += M_PI;
+        thm[a] = r; order[a] = a;
+    }
+    std::sort(order.begin(), order.end(), [&](int a, int b) { return thm[a] < thm[b]; });
+    for (int k = 0; k < na; ++k) { css[k] = cs[order[k]]; ths[k] = (float)thm[order[k]]; }
+    cudaError_t e = cudaSuccess;
+    auto twg = twiddles(G), twd = twiddles(nd);
+    if (e == cudaSuccess) e = upload(&p->twG, twg);
+    if (e == cudaSuccess) e = upload(&p->twD, twd);
+    if (e == cudaSuccess) e = upload(&p->ph_fwd, phf);
+    if (e == cudaSuccess) e = upload(&p->ph_adj, pha);
+    if (e == cudaSuccess) e = upload(&p->deapod, deapod);
+    if (e == cudaSuccess) e = upload(&p->cs, cs);
+    if (e == cudaSuccess) e = upload(&p->cs_sorted, css);
+    if (e == cudaSuccess) e = upload(&p->th_sorted, ths);
+    if (e == cudaSuccess) e = upload(&p->a_sorted, order);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&p->acc, (16 + 4096) * sizeof(double));
+    if (e != cudaSuccess) { tc_plan_destroy(p); return fail(e == cudaErrorMemoryAllocation ? TC_ENOMEM : TC_ECUDA, cudaGetErrorString(e)); }
+    d.twG = p->twG; d.twD = p->twD; d.ph_fwd = p->ph_fwd; d.ph_adj = p->ph_adj; d.deapod = p->deapod;
+    d.cs = p->cs; d.cs_sorted = p->cs_sorted; d.th_sorted = p->th_sorted; d.a_sorted = p->a_sorted;
+    *out = p;
+    return TC_OK;
+}
+
+static void free_scratch(tc_plan *p) {
+    cudaFree(p->rowbuf); cudaFree(p->grid); cudaFree(p->cpol);
+    p->rowbuf = p->grid = p->cpol = nullptr; p->ng_alloc = 0;
+    for (int b = 0; b < 2; ++b) { cudaFree(p->stage_in[b]); cudaFree(p->stage_out[b]); p->stage_in[b] = p->stage_out[b] = nullptr; }
+    p->stage_in_elems = p->stage_out_elems = 0;
+}
+
+extern "C" tc_status tc_plan_destroy(tc_plan *p) {
+    if (!p) return TC_OK;
+    free_scratch(p);
+    cudaFree(p->twG); cudaFree(p->twD); cudaFree(p->ph_fwd); cudaFree(p->ph_adj); cudaFree(p->deapod);
+    cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc);
+    if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
+    if (p->s_comp) cudaStreamDestroy(p->s_comp);
+    if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
+    delete p;
+    return TC_OK;
+}
+
+// bytes of scratch per group of 8 slices
+static size_t group_bytes(const tc_plan *p) {
+    const DevPlan &d = p->d;
+    return ((size_t)d.G * d.G + (size_t)d.n * d.G + (size_t)d.na * d.nd) * P * sizeof(float2);
+}
+
+// Decide the slab size (slices per pass through the pipeline) and allocate scratch for it.
+static tc_status ensure_scratch(tc_plan *p, int n_slices, int *slab_out) {
+    int want = (n_slices + 7) / 8;                                   // groups
+    if (p->max_slab) want = std::min(want, p->max_slab / 8);
+    if (want <= p->ng_alloc) { *slab_out = p->ng_alloc * 8; return TC_OK; }
+    if (p->ng_alloc == 0 || want > p->ng_alloc) {
+        size_t fr = 0, tot = 0;
+        CU(cudaMemGetInfo(&fr, &tot));
+        size_t have = (size_t)p->ng_alloc * group_bytes(p);
+        size_t budget = (size_t)((fr + have) * 0.45);
+        int fit = (int)std::max<size_t>(1, budget / group_bytes(p));
+        want = std::min(want, fit);
+        if (want <= p->ng_alloc) { *slab_out = p->ng_alloc * 8; return TC_OK; }
+        cudaFree(p->rowbuf); cudaFree(p->grid); cudaFree(p->cpol);
+        p->rowbuf = p->grid = p->cpol = nullptr; p->ng_alloc = 0;
+        const DevPlan &d = p->d;
+        CU(cudaMalloc((void **)&p->grid, (size_t)want * d.G * d.G * P * sizeof(float2)));
+        CU(cudaMalloc((void **)&p->rowbuf, (size_t)want * d.n * d.G * P * sizeof(float2)));
+        CU(cudaMalloc((void **)&p->cpol, (size_t)want * d.na * d.nd * P * sizeof(float2)));
+        p->ng_alloc = want;
+    }
+    *slab_out = p->ng_alloc * 8;
+    return TC_OK;
+}
+
+// ---- device pipelines (one slab, device pointers) ---------------------------------------------------
+static void forward_slab(tc_plan *p, const float *vol, int S, float *sino, cudaStream_t st) {
+    const int ng = (S + 7) / 8;
+    launch_fwd_rows(p->d, vol, S, ng, p->rowbuf, st);
+    launch_fwd_cols(p->d, p->rowbuf, ng, p->grid, st);
+    launch_fwd_gather(p->d, p->grid, S, ng, sino, st);
+}
+static void adjoint_slab(tc_plan *p, const float *sino, int S, float *vol, cudaStream_t st) {
+    const int ng = (S + 7) / 8;
+    launch_adj_radial(p->d, sino, S, ng, p->cpol, st);
+    launch_adj_spread(p->d, p->cpol, ng, p->grid, st);
+    launch_adj_cols(p->d, p->grid, ng, p->rowbuf, st);
+    launch_adj_rows(p->d, p->rowbuf, S, ng, vol, st);
+}
+
+static tc_status check_launch() {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(TC_ECUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
+    return TC_OK;
+}
+
+static bool is_device_ptr(const void *ptr) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, ptr) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+#include "tc_api_part2.inc"
