@@ -1,0 +1,264 @@
+#!/usr/bin/env python
+"""bench.py -- slice.projection pairs/s per MBIR iteration (forward + adjoint) on BASELINE config 4, 1xB200.
+
+A step = one pass of the whole hot path over one batch: tc_radon (F1-F4) then tc_backproject (B1-B4) on
+128 slices of 2048^2 with 1024 angles (centre 1027.5), device-resident.  `value` = S * Na * n_gpus / step time.
+`e2e` = the same through the C-ABI call with pinned HOST buffers (slab scheduler: H2D, compute, D2H inside the
+timed region).  `--impl reference` times the oracle (oracle/nufft.py, float64 numpy) on host cores instead.
+Prints ONE JSON line on rank 0.
+"""
+import argparse, json, os, subprocess, sys, threading, time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+METRIC = "slice_projection_pairs_per_s_fwd_adj"
+UNIT = "slice*projection pairs/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE config number (4 = the metric's workload)")
+    ap.add_argument("--slices", type=int, default=0, help="override slice count (debug)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--mbir", action="store_true", help="also time one MBIR iteration (extra.mbir_*)")
+    return ap.parse_args()
+
+
+def peak_hbm():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True); self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm = sorted(float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit())
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(len(r) > 3 + k and r[3 + k].lower().startswith("active") for r in self.rows)]
+        mx = next((float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()), None)
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": reasons, "samples": len(sm)}
+
+
+def stage_bytes(n, nd, na, S):
+    """algorithmic HBM bytes per launch of each kernel, S slices = ceil(S/8) groups of 32-byte cells."""
+    ng = (S + 7) // 8
+    G = 2 * n
+    cell = 32
+    return {
+        "fwd_rows": S * n * n * 4 + ng * n * G * cell,
+        "fwd_cols": ng * (n * G + G * G) * cell,
+        "fwd_gather": ng * G * G * cell + S * na * nd * 4,
+        "adj_radial": S * na * nd * 4 + ng * na * nd * cell,
+        "adj_spread": ng * na * nd * cell + ng * G * G * cell,
+        "adj_cols": ng * (G * G + n * G) * cell,
+        "adj_rows": ng * n * G * cell + S * n * n * 4,
+    }
+
+
+def oracle_sample(c, n_angles_sample):
+    """times oracle forward + adjoint of ONE slice on every (Na / n_angles_sample)-th angle; returns (pairs, seconds)."""
+    import numpy as np
+    from oracle import nufft
+    from paper_2304_12934_b200 import inputs
+    ang = inputs.angles_uniform(c["Na"]).astype(np.float64)[:: max(1, c["Na"] // n_angles_sample)]
+    vol = inputs.volume_fibres(1, c["N"], c["seed"], n_fibres=3000 if c["N"] >= 2048 else 300)[0]
+    t0 = time.perf_counter()
+    s = nufft.radon_nufft(vol, ang, c["Nd"], c["centre"])
+    nufft.backproject_nufft(s, ang, c["N"], c["centre"])
+    return len(ang), time.perf_counter() - t0
+
+
+def run_reference(args, c):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    nsel = 128
+    for _ in range(args.warmup):
+        oracle_sample(c, nsel)
+    tot, pairs = 0.0, 0
+    for _ in range(args.steps):
+        p, t = oracle_sample(c, nsel)
+        tot += t; pairs += p
+    val = pairs / tot
+    sample = "1 slice x %d of %d angles (every %dth), %dx%d, oracle/nufft.py forward+adjoint, float64 numpy" % (nsel, c["Na"], c["Na"] // nsel, c["N"], c["N"])
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config4: 128 slices 2048x2048, 1024 angles, 2048 bins, centre 1027.5 (bounded sample per step: %s)" % sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    args = parse()
+    from paper_2304_12934_b200 import inputs
+    c = dict(inputs.CONFIGS[args.config])
+    if args.slices:
+        c["S"] = args.slices
+    if args.impl == "reference":
+        return run_reference(args, c)
+
+    import numpy as np, torch, torch.distributed as dist
+    from paper_2304_12934_b200 import binding as tc
+    from paper_2304_12934_b200.shard import max_over_ranks
+    world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    S, N, Nd, Na = c["S"], c["N"], c["Nd"], c["Na"]
+    ang = inputs.angles_uniform(Na)
+    # weak scaling: every rank runs the whole config on its own z-range of a (world x S)-slice job; no data-path collective
+    nw = min(32, os.cpu_count() or 1)
+    if args.config == 4:
+        vol_h = inputs.volume_fibres(S, N, c["seed"] + rank, workers=nw)
+    elif args.config == 3:
+        vol_h = inputs.volume_porous(S, N, c["seed"] + rank)
+    elif args.config == 2:
+        vol_h = inputs.volume_cfg2()
+    else:
+        vol_h = inputs.volume_cfg1() if args.config == 1 else inputs.volume_fibres(S, N, c["seed"], workers=nw)
+    plan = tc.Plan(N, Nd, ang, c["centre"])
+    vol = torch.from_numpy(vol_h).cuda()
+    sino = torch.empty((S, Na, Nd), dtype=torch.float32, device="cuda")
+    back = torch.empty_like(vol)
+
+    def step():
+        plan.radon(vol, out=sino)
+        plan.backproject(sino, out=back)
+
+    def fence():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 1)):
+        step()
+    fence()
+    plan.profile(True); plan.profile_read(); tc.launch_count(reset=True)
+    sampler = ClockSampler(local); sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    fence()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    fence()
+    secs = max_over_ranks(e0.elapsed_time(e1) * 1e-3)
+    clocks = sampler.stop()
+    launches = tc.launch_count()
+    stages = plan.profile_read(); plan.profile(False)
+    ms_step = 1e3 * secs / args.steps
+    value = world * S * Na / (secs / args.steps)
+
+    peak, peak_src = peak_hbm()
+    sb = stage_bytes(N, Nd, Na, S)
+    per = {k: (ms / max(cnt, 1), cnt) for k, (ms, cnt) in stages.items()}
+    dom = max(per, key=lambda k: per[k][0] * per[k][1])
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            traffic = json.load(fh).get("config%d" % args.config, {}).get(dom)
+    except Exception:
+        pass
+    ach = sb[dom] / (per[dom][0] * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": traffic,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": sb[dom], "avg_launch_ms": per[dom][0]}
+    model_bytes = (104 * N * N + 8 * Na * Nd) * S           # fwd+adj staged-byte model per slice
+    extra = {"stage_ms_per_step": {k: per[k][0] * per[k][1] / args.steps for k in per},
+             "stage_GBps": {k: sb[k] / (per[k][0] * 1e-3) / 1e9 if per[k][0] > 0 else None for k in per},
+             "fwd_pairs_per_s": S * Na / (sum(per[k][0] * per[k][1] for k in per if k.startswith("fwd")) / args.steps * 1e-3),
+             "adj_pairs_per_s": S * Na / (sum(per[k][0] * per[k][1] for k in per if k.startswith("adj")) / args.steps * 1e-3),
+             "step_model_bytes": model_bytes, "step_frac_of_hbm_roofline": model_bytes / (secs / args.steps) / 1e9 / peak,
+             "step_frac_of_nominal_8TBs": model_bytes / (secs / args.steps) / 8e12}
+
+    # ---- e2e: host buffers through the C ABI (slab scheduler) ----
+    e2e = None
+    if not args.no_e2e:
+        hv = torch.from_numpy(vol_h).pin_memory()
+        hs = torch.empty((S, Na, Nd), dtype=torch.float32).pin_memory()
+        hb = torch.empty((S, N, N), dtype=torch.float32).pin_memory()
+        plan.radon(hv, out=hs); plan.backproject(hs, out=hb)      # warm-up (allocates staging)
+        fence()
+        t0 = time.perf_counter()
+        ov = []
+        for _ in range(args.steps):
+            plan.radon(hv, out=hs); ov.append(plan.sched_stats()["overlap"])
+            plan.backproject(hs, out=hb); ov.append(plan.sched_stats()["overlap"])
+        fence()
+        t_e2e = max_over_ranks(time.perf_counter() - t0)
+        bytes_in = hv.numel() * 4 + hs.numel() * 4
+        bytes_out = hs.numel() * 4 + hb.numel() * 4
+        e2e = {"value": world * S * Na / (t_e2e / args.steps), "unit": UNIT, "h2d_bytes_per_step": bytes_in, "d2h_bytes_per_step": bytes_out,
+               "ms_per_step": 1e3 * t_e2e / args.steps, "pcie_GBps": (bytes_in + bytes_out) / (t_e2e / args.steps) / 1e9,
+               "overlap_mean": float(np.mean(ov))}
+        del hv, hs, hb
+
+    if args.mbir:
+        Sm = min(S, 32)
+        b = sino[:Sm].contiguous()
+        pr = tc.prior_params(L=float(1.05 * 1.02 * Na * N + 4.0 / (1e-4 * (1 / 0.7) ** 2)))
+        plan.mbir(b, pr, 1); fence()
+        t0 = time.perf_counter(); plan.mbir(b, pr, 1); fence(); t1 = time.perf_counter() - t0
+        t0 = time.perf_counter(); plan.mbir(b, pr, 4); fence(); t4 = time.perf_counter() - t0
+        extra["mbir_iter_ms"] = 1e3 * (t4 - t1) / 3
+        extra["mbir_pairs_per_s"] = Sm * Na / ((t4 - t1) / 3)
+        extra["mbir_slices"] = Sm
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        nsel = 512 if Na >= 512 else Na
+        pairs, t = oracle_sample(c, nsel)
+        cpu = {"value": pairs / t, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": "1 slice x %d of %d angles, %dx%d, oracle/nufft.py forward+adjoint (float64 numpy, single thread), %.1f s" % (pairs, Na, N, N, t)}
+    plan.close()
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "config%d: %d slices %dx%d float32 fibre-composite phantom (seed %d), %d angles in [0,pi), %d bins, centre %.1f, oversampling 2, KB width 6; step = tc_radon + tc_backproject"
+                       % (args.config, S, N, N, c["seed"], Na, Nd, c["centre"]),
+                       "l2": "inputs larger than L2 (volume %.2f GB, sinogram %.2f GB, fine grid %.1f GB per step)" % (S * N * N * 4e-9, S * Na * Nd * 4e-9, ((S + 7) // 8) * 4 * N * N * 32e-9),
+                       "parallelism": "z-shards, no collective (x%d)" % world},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "extra": extra}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

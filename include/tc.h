@@ -30,7 +30,7 @@ typedef enum { TC_OK = 0, TC_EINVAL = 1, TC_ENOMEM = 2, TC_ECUDA = 3, TC_EUNSUPP
 /* Acquisition geometry.  n: image side (even); n_det: detector bins (even); angles: HOST pointer to
  * n_angles float32 radians (copied at plan creation; any finite values); center: rotation-axis
  * position in bins (< 0 means n_det/2); oversamp must be 2.0 and kb_width 6 (Kaiser-Bessel
- * window; w ~ log10(1/eps)).  2n and n_det must factor into {2, 3, 5}. */
+ * window; w ~ log10(1/eps)).  n must be a multiple of 32; 2n and n_det must be 2^a 5^b with b <= 1 (else TC_EUNSUPPORTED). */
 typedef struct {
     int n, n_det, n_angles;
     const float *angles;
@@ -87,6 +87,14 @@ long long tc_launch_count(int reset);
  * spans) and wall; overlap = (copy + compute - wall) / min(copy, compute). */
 typedef struct { double h2d_s, compute_s, d2h_s, wall_s, overlap; long long h2d_bytes, d2h_bytes; int n_slabs; } tc_sched_stats;
 tc_status tc_last_sched_stats(tc_plan *plan, tc_sched_stats *out);
+
+/* Per-kernel timing with CUDA events recorded on the launching stream around every NUFFT stage launch
+ * (stages: 0 fwd_rows, 1 fwd_cols, 2 fwd_gather, 3 adj_radial, 4 adj_spread, 5 adj_cols, 6 adj_rows).
+ * tc_profile switches recording on/off; tc_profile_read waits for the recorded events, returns summed
+ * milliseconds and launch counts per stage (arrays of TC_N_STAGES, HOST) and clears the records. */
+#define TC_N_STAGES 7
+tc_status tc_profile(tc_plan *plan, int enable);
+tc_status tc_profile_read(tc_plan *plan, double *ms, long long *launches);
 
 const char *tc_last_error(void);
 

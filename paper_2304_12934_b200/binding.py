@@ -49,9 +49,11 @@ lib.tc_radon1.argtypes = [_vp, _ci, _ci, ctypes.POINTER(ctypes.c_float), _ci, _c
 lib.tc_launch_count.argtypes = [_ci]
 lib.tc_launch_count.restype = ctypes.c_longlong
 lib.tc_last_sched_stats.argtypes = [_vp, ctypes.POINTER(tc_sched_stats)]
+lib.tc_profile.argtypes = [_vp, _ci]
+lib.tc_profile_read.argtypes = [_vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_longlong)]
 lib.tc_last_error.restype = ctypes.c_char_p
 for _f in ("tc_plan_create", "tc_plan_destroy", "tc_radon", "tc_backproject", "tc_mbir", "tc_power_iteration",
-           "tc_prior_eval", "tc_radon1", "tc_last_sched_stats"):
+           "tc_prior_eval", "tc_radon1", "tc_last_sched_stats", "tc_profile", "tc_profile_read"):
     getattr(lib, _f).restype = _ci
 
 
@@ -138,6 +140,16 @@ class Plan:
         v = ctypes.c_double()
         _check(lib.tc_power_iteration(self._h, int(iters), ctypes.byref(v)))
         return v.value
+
+    STAGES = ("fwd_rows", "fwd_cols", "fwd_gather", "adj_radial", "adj_spread", "adj_cols", "adj_rows")
+
+    def profile(self, enable=True):
+        _check(lib.tc_profile(self._h, 1 if enable else 0))
+
+    def profile_read(self):
+        ms = (ctypes.c_double * 7)(); cnt = (ctypes.c_longlong * 7)()
+        _check(lib.tc_profile_read(self._h, ms, cnt))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(self.STAGES)}
 
     def sched_stats(self):
         s = tc_sched_stats()

@@ -46,7 +46,24 @@ struct tc_plan {
     size_t stage_in_elems = 0, stage_out_elems = 0;
     cudaStream_t s_h2d = nullptr, s_comp = nullptr, s_d2h = nullptr;
     tc_sched_stats stats{};
+    // per-stage CUDA-event timing (tc_profile)
+    bool prof = false;
+    struct ProfRec { int stage; cudaEvent_t a, b; };
+    std::vector<ProfRec> prof_recs;
 };
+
+static void prof_stage(tc_plan *p, int stage, cudaStream_t st, bool begin) {
+    if (!p->prof) return;
+    if (begin) {
+        tc_plan::ProfRec r; r.stage = stage;
+        cudaEventCreate(&r.a); cudaEventCreate(&r.b);
+        cudaEventRecord(r.a, st);
+        p->prof_recs.push_back(r);
+    } else {
+        cudaEventRecord(p->prof_recs.back().b, st);
+    }
+}
+#define STAGE(id, call) do { prof_stage(p, id, st, true); call; prof_stage(p, id, st, false); } while (0)
 
 // ---- host-side mathematics of the plan (float64) ---------------------------------------------------
 static double bessel_i0(double x) {          // I0(x) = sum_k (x^2/4)^k / (k!)^2
@@ -230,16 +247,35 @@ static tc_status ensure_scratch(tc_plan *p, int n_slices, int *slab_out) {
 // ---- device pipelines (one slab, device pointers) ---------------------------------------------------
 static void forward_slab(tc_plan *p, const float *vol, int S, float *sino, cudaStream_t st) {
     const int ng = (S + 7) / 8;
-    launch_fwd_rows(p->d, vol, S, ng, p->rowbuf, st);
-    launch_fwd_cols(p->d, p->rowbuf, ng, p->grid, st);
-    launch_fwd_gather(p->d, p->grid, S, ng, sino, st);
+    STAGE(0, launch_fwd_rows(p->d, vol, S, ng, p->rowbuf, st));
+    STAGE(1, launch_fwd_cols(p->d, p->rowbuf, ng, p->grid, st));
+    STAGE(2, launch_fwd_gather(p->d, p->grid, S, ng, sino, st));
 }
 static void adjoint_slab(tc_plan *p, const float *sino, int S, float *vol, cudaStream_t st) {
     const int ng = (S + 7) / 8;
-    launch_adj_radial(p->d, sino, S, ng, p->cpol, st);
-    launch_adj_spread(p->d, p->cpol, ng, p->grid, st);
-    launch_adj_cols(p->d, p->grid, ng, p->rowbuf, st);
-    launch_adj_rows(p->d, p->rowbuf, S, ng, vol, st);
+    STAGE(3, launch_adj_radial(p->d, sino, S, ng, p->cpol, st));
+    STAGE(4, launch_adj_spread(p->d, p->cpol, ng, p->grid, st));
+    STAGE(5, launch_adj_cols(p->d, p->grid, ng, p->rowbuf, st));
+    STAGE(6, launch_adj_rows(p->d, p->rowbuf, S, ng, vol, st));
+}
+
+extern "C" tc_status tc_profile(tc_plan *p, int enable) {
+    if (!p) return fail(TC_EINVAL, "null plan");
+    p->prof = enable != 0;
+    return TC_OK;
+}
+extern "C" tc_status tc_profile_read(tc_plan *p, double *ms, long long *launches) {
+    if (!p || !ms || !launches) return fail(TC_EINVAL, "null argument");
+    for (int i = 0; i < TC_N_STAGES; ++i) { ms[i] = 0.0; launches[i] = 0; }
+    for (auto &r : p->prof_recs) {
+        float t = 0.f;
+        CU(cudaEventSynchronize(r.b));
+        CU(cudaEventElapsedTime(&t, r.a, r.b));
+        ms[r.stage] += t; launches[r.stage] += 1;
+        cudaEventDestroy(r.a); cudaEventDestroy(r.b);
+    }
+    p->prof_recs.clear();
+    return TC_OK;
 }
 
 static tc_status check_launch() {

@@ -89,30 +89,42 @@ def volume_porous(S, n, seed, n_pores=400, rmin=4.0, rmax=40.0):
     return vol
 
 
-def volume_fibres(S, n, seed, n_fibres=3000):
-    """cfg 4: matrix density 0.1 inside radius 0.47 N; cylinders within 15 deg of z, radii U(3,12) px
-    (scaled by n/2048), density U(0.2, 1.0); a slice cuts each as an ellipse."""
+def _fibre_params(n, seed, n_fibres):
     rng = np.random.default_rng(seed)
-    x = np.arange(n) - n // 2
-    base = 0.1 * ((x[None, :] ** 2 + x[:, None] ** 2) <= (0.47 * n) ** 2)
     scale = n / 2048.0
     r = 0.44 * n * np.sqrt(rng.random(n_fibres)); ang = rng.random(n_fibres) * 2 * np.pi
-    cx, cy = r * np.cos(ang), r * np.sin(ang)
-    tilt = np.deg2rad(rng.uniform(0, 15, n_fibres)); az = rng.random(n_fibres) * 2 * np.pi
-    R = rng.uniform(3, 12, n_fibres) * scale
-    rho = rng.uniform(0.2, 1.0, n_fibres)
-    vol = np.empty((S, n, n), dtype=np.float32)
-    for z in range(S):
-        img = base.copy()
-        dz = z - S / 2
-        for k in range(n_fibres):
-            sx = cx[k] + dz * np.tan(tilt[k]) * np.cos(az[k])
-            sy = cy[k] + dz * np.tan(tilt[k]) * np.sin(az[k])
-            if np.hypot(sx, sy) + R[k] / np.cos(tilt[k]) > 0.47 * n:
-                continue
-            _add_ellipse(img, sx, sy, R[k] / np.cos(tilt[k]), R[k], az[k], rho[k])
-        vol[z] = img
-    return vol
+    return dict(cx=r * np.cos(ang), cy=r * np.sin(ang), tilt=np.deg2rad(rng.uniform(0, 15, n_fibres)),
+                az=rng.random(n_fibres) * 2 * np.pi, R=rng.uniform(3, 12, n_fibres) * scale, rho=rng.uniform(0.2, 1.0, n_fibres))
+
+
+def _fibre_slice(args):
+    z, S, n, seed, n_fibres = args
+    q = _fibre_params(n, seed, n_fibres)
+    x = np.arange(n) - n // 2
+    img = 0.1 * ((x[None, :] ** 2 + x[:, None] ** 2) <= (0.47 * n) ** 2)
+    dz = z - S / 2
+    for k in range(n_fibres):
+        sx = q["cx"][k] + dz * np.tan(q["tilt"][k]) * np.cos(q["az"][k])
+        sy = q["cy"][k] + dz * np.tan(q["tilt"][k]) * np.sin(q["az"][k])
+        a = q["R"][k] / np.cos(q["tilt"][k])
+        if np.hypot(sx, sy) + a > 0.47 * n:
+            continue
+        _add_ellipse(img, sx, sy, a, q["R"][k], q["az"][k], q["rho"][k])
+    return img.astype(np.float32)
+
+
+def volume_fibres(S, n, seed, n_fibres=3000, workers=1):
+    """cfg 4: matrix density 0.1 inside radius 0.47 N; cylinders within 15 deg of z, radii U(3,12) px
+    (scaled by n/2048), density U(0.2, 1.0); a slice cuts each as an ellipse.  Slices are independent given the
+    seed, so `workers` > 1 rasterises them in a process pool (same result)."""
+    jobs = [(z, S, n, seed, n_fibres) for z in range(S)]
+    if workers > 1:
+        import multiprocessing as mp
+        with mp.get_context("fork").Pool(workers) as pool:
+            sl = pool.map(_fibre_slice, jobs, chunksize=max(1, S // (4 * workers)))
+    else:
+        sl = [_fibre_slice(j) for j in jobs]
+    return np.stack(sl)
 
 
 def poisson_sinogram(sino, seed, photons=1e4, peak=2.0):
