@@ -9,6 +9,8 @@ constexpr int KB_W = 6;          // Kaiser-Bessel window width (taps per axis)
 constexpr int KB_DEG = 12;       // degree of the window polynomial in z = 2 q - 1, q = 1 - (2 r / W)^2
 constexpr int P = 4;             // complex planes interleaved per fine-grid cell (= 8 real slices, 32 B)
 
+struct TileRange { int start, count, shx, shy; };   // angles (sorted order) whose ray can touch a 32 x 8 tile, per wrap alias
+
 // Everything the kernels need, passed by value.
 struct DevPlan {
     int n, nd, na, G;
@@ -22,6 +24,9 @@ struct DevPlan {
     const double2 *cs_sorted;     // [na] same, sorted by theta mod pi
     const float *th_sorted;       // [na] theta mod pi, ascending
     const int *a_sorted;          // [na] original angle index
+    const TileRange *tile_rng;    // [tiles][4]
+    const int *tile_nr;           // [tiles] number of valid ranges
+    int J;                        // radial modes to try on each side of the nearest one: floor(3 sqrt2 / sc + 1/2)
 };
 
 // Window polynomial coefficients (monomial in z, c[0] + c[1] z + ...), set by the plan.
@@ -37,6 +42,7 @@ void launch_fwd_gather(const DevPlan &d, const float2 *grid, int S, int ng, floa
 // sino -> cpol [ng][na][nd][P] c64               (B1 radial FFT + conjugate phase)
 void launch_adj_radial(const DevPlan &d, const float *sino, int S, int ng, float2 *cpol, cudaStream_t st);
 // cpol -> grid                                   (B2 spread, evaluated per fine-grid cell: plain stores, no atomics)
+void launch_tile_ranges(const DevPlan &d, TileRange *rng, int *nrng, cudaStream_t st);
 void launch_adj_spread(const DevPlan &d, const float2 *cpol, int ng, float2 *grid, cudaStream_t st);
 // grid -> rowbuf (cropped to n rows)             (B3 inverse column FFT)
 void launch_adj_cols(const DevPlan &d, const float2 *grid, int ng, float2 *rowbuf, cudaStream_t st);

@@ -36,7 +36,8 @@ struct tc_plan {
     float2 *twG = nullptr, *twD = nullptr, *ph_fwd = nullptr, *ph_adj = nullptr;
     float *deapod = nullptr, *th_sorted = nullptr;
     double2 *cs = nullptr, *cs_sorted = nullptr;
-    int *a_sorted = nullptr;
+    int *a_sorted = nullptr, *tile_nr = nullptr;
+    TileRange *tile_rng = nullptr;
     // scratch
     int ng_alloc = 0;
     float2 *rowbuf = nullptr, *grid = nullptr, *cpol = nullptr;
@@ -190,6 +191,17 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
     if (e != cudaSuccess) { tc_plan_destroy(p); return fail(e == cudaErrorMemoryAllocation ? TC_ENOMEM : TC_ECUDA, cudaGetErrorString(e)); }
     d.twG = p->twG; d.twD = p->twD; d.ph_fwd = p->ph_fwd; d.ph_adj = p->ph_adj; d.deapod = p->deapod;
     d.cs = p->cs; d.cs_sorted = p->cs_sorted; d.th_sorted = p->th_sorted; d.a_sorted = p->a_sorted;
+    d.J = (int)std::floor(3.0 * std::sqrt(2.0) / d.sc + 0.5);
+    {
+        const int nt = ((G + 31) / 32) * ((G + 7) / 8);
+        e = cudaMalloc((void **)&p->tile_rng, (size_t)nt * 4 * sizeof(TileRange));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&p->tile_nr, (size_t)nt * sizeof(int));
+        if (e != cudaSuccess) { tc_plan_destroy(p); return fail(TC_ENOMEM, cudaGetErrorString(e)); }
+        d.tile_rng = p->tile_rng; d.tile_nr = p->tile_nr;
+        launch_tile_ranges(d, p->tile_rng, p->tile_nr, nullptr);
+        e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) { tc_plan_destroy(p); return fail(TC_ECUDA, std::string("tile ranges: ") + cudaGetErrorString(e)); }
+    }
     *out = p;
     return TC_OK;
 }
@@ -205,7 +217,7 @@ extern "C" tc_status tc_plan_destroy(tc_plan *p) {
     if (!p) return TC_OK;
     free_scratch(p);
     cudaFree(p->twG); cudaFree(p->twD); cudaFree(p->ph_fwd); cudaFree(p->ph_adj); cudaFree(p->deapod);
-    cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc);
+    cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc); cudaFree(p->tile_rng); cudaFree(p->tile_nr);
     if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
     if (p->s_comp) cudaStreamDestroy(p->s_comp);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
