@@ -26,6 +26,8 @@ struct DevPlan {
     const int *a_sorted;          // [na] original angle index
     const TileRange *tile_rng;    // [tiles][4]
     const int *tile_nr;           // [tiles] number of valid ranges
+    const unsigned *tap_offs;     // [tiles * 256 + 1] CSR offsets of the spread's per-cell tap lists (cell order: tile, then thread)
+    const int2 *taps;             // (a * nd + (m mod nd), float weight bits)
     int J;                        // radial modes to try on each side of the nearest one: floor(3 sqrt2 / sc + 1/2)
 };
 
@@ -43,6 +45,8 @@ void launch_fwd_gather(const DevPlan &d, const float2 *grid, int S, int ng, floa
 void launch_adj_radial(const DevPlan &d, const float *sino, int S, int ng, float2 *cpol, cudaStream_t st);
 // cpol -> grid                                   (B2 spread, evaluated per fine-grid cell: plain stores, no atomics)
 void launch_tile_ranges(const DevPlan &d, TileRange *rng, int *nrng, cudaStream_t st);
+void launch_spread_count(const DevPlan &d, int *counts, cudaStream_t st);
+void launch_spread_fill(const DevPlan &d, cudaStream_t st);
 void launch_adj_spread(const DevPlan &d, const float2 *cpol, int ng, float2 *grid, cudaStream_t st);
 // grid -> rowbuf (cropped to n rows)             (B3 inverse column FFT)
 void launch_adj_cols(const DevPlan &d, const float2 *grid, int ng, float2 *rowbuf, cudaStream_t st);

@@ -9,6 +9,7 @@
 #include <algorithm>
 #include "../../include/tc.h"
 #include "common.cuh"
+#include <cub/device/device_scan.cuh>
 
 using namespace tc;
 
@@ -38,6 +39,9 @@ struct tc_plan {
     double2 *cs = nullptr, *cs_sorted = nullptr;
     int *a_sorted = nullptr, *tile_nr = nullptr;
     TileRange *tile_rng = nullptr;
+    unsigned *tap_offs = nullptr;
+    int2 *taps = nullptr;
+    long long n_taps = 0;
     // scratch
     int ng_alloc = 0;
     float2 *rowbuf = nullptr, *grid = nullptr, *cpol = nullptr;
@@ -201,6 +205,28 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
         launch_tile_ranges(d, p->tile_rng, p->tile_nr, nullptr);
         e = cudaDeviceSynchronize();
         if (e != cudaSuccess) { tc_plan_destroy(p); return fail(TC_ECUDA, std::string("tile ranges: ") + cudaGetErrorString(e)); }
+        // per-cell tap lists of the spread (B2): count, exclusive scan (cub), fill
+        const size_t nc = (size_t)nt * 256;
+        int *counts = nullptr; void *tmp = nullptr; size_t tmp_bytes = 0;
+        e = cudaMalloc((void **)&counts, (nc + 1) * sizeof(int));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&p->tap_offs, (nc + 1) * sizeof(unsigned));
+        if (e == cudaSuccess) e = cudaMemset(counts, 0, (nc + 1) * sizeof(int));
+        if (e == cudaSuccess) {
+            launch_spread_count(d, counts, nullptr);
+            cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, (const unsigned *)counts, p->tap_offs, (int)(nc + 1));
+            e = cudaMalloc(&tmp, tmp_bytes);
+        }
+        if (e == cudaSuccess) e = cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, (const unsigned *)counts, p->tap_offs, (int)(nc + 1));
+        unsigned total = 0;
+        if (e == cudaSuccess) e = cudaMemcpy(&total, p->tap_offs + nc, sizeof(unsigned), cudaMemcpyDeviceToHost);
+        cudaFree(counts); cudaFree(tmp);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&p->taps, (size_t)std::max(total, 1u) * sizeof(int2));
+        if (e != cudaSuccess) { tc_plan_destroy(p); return fail(e == cudaErrorMemoryAllocation ? TC_ENOMEM : TC_ECUDA, std::string("spread tap lists: ") + cudaGetErrorString(e)); }
+        p->n_taps = total;
+        d.tap_offs = p->tap_offs; d.taps = p->taps;
+        launch_spread_fill(d, nullptr);
+        e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) { tc_plan_destroy(p); return fail(TC_ECUDA, std::string("spread tap lists: ") + cudaGetErrorString(e)); }
     }
     *out = p;
     return TC_OK;
@@ -217,7 +243,7 @@ extern "C" tc_status tc_plan_destroy(tc_plan *p) {
     if (!p) return TC_OK;
     free_scratch(p);
     cudaFree(p->twG); cudaFree(p->twD); cudaFree(p->ph_fwd); cudaFree(p->ph_adj); cudaFree(p->deapod);
-    cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc); cudaFree(p->tile_rng); cudaFree(p->tile_nr);
+    cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc); cudaFree(p->tile_rng); cudaFree(p->tile_nr); cudaFree(p->tap_offs); cudaFree(p->taps);
     if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
     if (p->s_comp) cudaStreamDestroy(p->s_comp);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
