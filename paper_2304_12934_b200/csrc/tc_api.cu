@@ -111,8 +111,9 @@ static bool make_fft_desc(int n, FftDesc &f) {
     int m = n, fives = 0, twos = 0;
     while (m % 5 == 0) { m /= 5; ++fives; }
     while (m % 2 == 0) { m /= 2; ++twos; }
-    if (m != 1 || fives > 1 || n < 8) return false;
+    if (m != 1 || fives > 1 || (twos % 3 != 0) + twos / 3 + fives < 2) return false;   // at least two passes
     f.n = n; f.ps = n + (n >> 4) + 1;
+    while (f.ps % 8 != 4) ++f.ps;                 // plane pairs of the two lanes of a thread pair land on complementary banks
     f.first = twos % 3 == 1 ? 2 : (twos % 3 == 2 ? 4 : 0);
     f.n8 = twos / 3; f.five = fives;
     return true;
