@@ -15,8 +15,8 @@ struct TileRange { int start, count, shx, shy; };   // angles (sorted order) who
 struct DevPlan {
     int n, nd, na, G;
     double sc;                    // G / nd: fine-grid cells per radial mode
-    FftDesc fG, fD;               // FFT descriptors for length G (fine grid) and nd (radial)
-    const float2 *twG, *twD;      // twiddles e^{-2 pi i k / n}
+    FftDesc fN, fD;               // FFT descriptors for length n (half of the fine grid: pruned split) and nd (radial)
+    const float2 *twG, *twD;      // twiddles e^{-2 pi i k / G} (length G; the length-n transforms use every 2nd) and e^{-2 pi i k / nd}
     const float *deapod;          // d(x_j) = 1 / phihat(x_j), j < n
     const float2 *ph_fwd;         // [nd] e^{-2 pi i m centre / nd} / nd, Nyquist entry 0 (forward, before the inverse radial FFT)
     const float2 *ph_adj;         // [nd] e^{+2 pi i m centre / nd} / nd, Nyquist entry 0 (adjoint, after the radial FFT)

@@ -1,165 +1,262 @@
-// Line FFT with the first pass fused into the global load and the last pass fused into the global store.
+// Line FFT engine: one CTA transforms one line of P = 4 complex planes (a line of 32-byte cells), length
+// n = R1 R2 ... RL, with the first pass fused into the load and the last pass fused into the store.
 //
-// One CTA transforms one line of P = 4 complex planes, length n = 2^a 5^b.  Thread t owns plane pair
-// pp = t & 1 (planes 2pp, 2pp+1 = one 16-byte half of a 32-byte cell) and butterfly slot bt = t >> 1, so the
-// two lanes of a pair touch the two halves of the same cell in the same instruction: every global access is
-// a whole sector.  Passes are Stockham autosort steps (see fft.cuh); only the passes in the middle go
-// shared -> shared.  E = butterfly elements a thread holds per plane (8: one radix-8 butterfly).
+// Thread t owns plane pl = t & 3 and task slot t >> 2: the four lanes of a quad touch the four 8-byte planes of
+// the same 32-byte cell in the same instruction, so every global access is a whole sector.  A task is one
+// radix-R butterfly of one plane, held in registers; tasks of a pass are independent, a thread runs any number
+// of them one after the other, and there is one barrier per pass.
 //
-//   first pass  (s = 1):  x[b + nb j] come from `ld(index)`;  y[R b + k] -> shared memory
-//   middle passes:        shared -> registers -> (barrier) -> shared
-//   last pass   (m = 1):  x[b + s j] from shared memory;  y[b + s k] go to `st(index, value)`
-//
-// ld(idx) returns float4 = (plane 2pp re, im, plane 2pp+1 re, im); st(idx, float4) stores the same.
+// Decimation in frequency with a transposing first pass, all later passes in place:
+//   first pass   task b < n/R1:  x[b + (n/R1) j] (from `ld`)  -> DFT over j -> * w_n^{b k1} -> cell R1 b + k1
+//   pass i       sub-transform of size n_i = n / (R1..R_{i-1}) inside every residue; task (outer, b_i, k1):
+//                cells R1 (outer n_i + j_i (n_i/R_i) + b_i) + k1, j_i < R_i, DFT over j_i in place,
+//                * w_{n_i}^{b_i k_i}
+//   last pass    (n_L = R_L, no twiddles) task T = k1 + R1 k2 + ...: outputs X[T + (n/R_L) k_L] go to `st`
+// Shared-memory cell c is stored at c + (c >> 4) (one padding cell per 16) so that the first pass's stride-R1
+// writes and every later consecutive-k1 access are free of bank conflicts with 8-byte lanes.
+// tw[i * tws] = e^{-2 pi i * i / n}.
 #pragma once
 #include "fft.cuh"
 
 namespace tc {
 
-struct LineCtx {
-    float2 *sm;               // P planes of stride ps
-    const float2 *tw;         // e^{-2 pi i k / n}
-    int n, ps, pp, bt, nbt;   // nbt = butterfly slots = blockDim.x / 2
-    float dir;
+constexpr int LINE_THREADS = 512;
+constexpr int LINE_SLOTS = LINE_THREADS / 4;
+
+__device__ __forceinline__ int pcell(int c) { return c + (c >> 4); }
+
+// Pass configuration: compile-time (every index, stride and radix folds to an immediate) for the sizes of the
+// BASELINE configs, run-time (from the descriptor) for everything else.  TWS = stride of the twiddle table.
+template <int N_, int TWS_, int... Rs> struct SCfg {
+    static constexpr bool is_static = true;
+    static constexpr int NP = sizeof...(Rs);
+    __device__ __forceinline__ static constexpr int n() { return N_; }
+    __device__ __forceinline__ static constexpr int tws() { return TWS_; }
+    __device__ __forceinline__ static constexpr int npass() { return NP; }
+    __device__ __forceinline__ static constexpr int radix(int i) { constexpr int r[NP] = {Rs...}; return r[i]; }
+};
+struct RCfg {
+    static constexpr bool is_static = false;
+    FftDesc d; int tws_;
+    __device__ __forceinline__ int n() const { return d.n; }
+    __device__ __forceinline__ int tws() const { return tws_; }
+    __device__ __forceinline__ int npass() const { return d.npass; }
+    __device__ __forceinline__ int radix(int i) const { return d.radix[i]; }
 };
 
-template <int R>
-__device__ __forceinline__ void line_twiddles(const LineCtx &c, int base, float2 (&w)[R]) {
-    w[1] = __ldg(&c.tw[base]);
-    if (R > 2) w[2] = __ldg(&c.tw[2 * base]);
-    if (R > 3) w[3] = cmul(w[1], w[2]);
-    if (R > 4) w[4] = __ldg(&c.tw[4 * base]);
-    if (R > 5) { w[5] = cmul(w[4], w[1]); w[6] = cmul(w[4], w[2]); w[7] = cmul(w[4], w[3]); }
-    if (c.dir > 0.f) {
-#pragma unroll
-        for (int k = 1; k < R; ++k) w[k].y = -w[k].y;
+struct LineCtx {
+    float2 *sm;               // [padded cell][4 planes]
+    const float2 *tw;
+    int pl, slot;
+};
+
+// v[k] *= w^k, w = tw[base * tws] (conjugated for the inverse); powers from tw[base], tw[2 base], tw[4 base], tw[8 base]
+template <int R, bool INV>
+__device__ __forceinline__ void twiddle_mul(const float2 *__restrict__ t, int e, float2 (&v)[R]) {
+    float2 w1 = __ldg(t + e);
+    if (INV) w1.y = -w1.y;
+    v[1] = cmul(v[1], w1);
+    if (R > 2) {
+        float2 w2 = __ldg(t + 2 * e); if (INV) w2.y = -w2.y;
+        const float2 w3 = cmul(w1, w2);
+        v[2] = cmul(v[2], w2); v[3] = cmul(v[3], w3);
+        if (R > 4) {
+            float2 w4 = __ldg(t + 4 * e); if (INV) w4.y = -w4.y;
+            const float2 w5 = cmul(w4, w1), w6 = cmul(w4, w2), w7 = cmul(w4, w3);
+            v[4] = cmul(v[4], w4); v[5] = cmul(v[5], w5); v[6] = cmul(v[6], w6); v[7] = cmul(v[7], w7);
+            if (R > 8) {
+                float2 w8 = __ldg(t + 8 * e); if (INV) w8.y = -w8.y;
+                v[8] = cmul(v[8], w8);
+                v[9] = cmul(v[9], cmul(w8, w1)); v[10] = cmul(v[10], cmul(w8, w2)); v[11] = cmul(v[11], cmul(w8, w3));
+                v[12] = cmul(v[12], cmul(w8, w4)); v[13] = cmul(v[13], cmul(w8, w5)); v[14] = cmul(v[14], cmul(w8, w6));
+                v[15] = cmul(v[15], cmul(w8, w7));
+            }
+        }
     }
 }
 
-template <int R, int E, class LD>
-__device__ __forceinline__ void line_first_pass(const LineCtx &c, LD ld) {
-    constexpr int MAXC = (E + R - 1) / R;
-    const int nb = c.n / R;
-    float2 *s0 = c.sm + (2 * c.pp) * c.ps, *s1 = s0 + c.ps;
-    float4 v[MAXC][R];
+// first pass: global (through ld) -> shared
+template <int R, bool INV, class Cfg, class LD>
+__device__ __forceinline__ void line_first(const LineCtx &c, const Cfg &cfg, LD ld) {
+    const int nb = cfg.n() / R;
+#pragma unroll 1
+    for (int b = c.slot; b < nb; b += LINE_SLOTS) {
+        float2 v[R];
 #pragma unroll
-    for (int cc = 0; cc < MAXC; ++cc) {
-        const int b = c.bt + cc * c.nbt;
-        if (b < nb) {
+        for (int j = 0; j < R; ++j) v[j] = ld(b + nb * j);
+        Bfly<R, INV>::run(v);
+        twiddle_mul<R, INV>(c.tw, b * cfg.tws(), v);
+        float2 *o = c.sm + pcell(R * b) * 4 + c.pl;   // R b is a multiple of R and R divides 16: k never crosses a padding cell
 #pragma unroll
-            for (int j = 0; j < R; ++j) v[cc][j] = ld(b + nb * j);
-        }
+        for (int k = 0; k < R; ++k) o[k * 4] = v[k];
     }
+    __syncthreads();
+}
+
+// first pass when the producer already left the line in shared memory: element t = b + (n/R) j at cell R b + j
+// (line_input_cell), transformed in place.
+__device__ __forceinline__ int line_input_cell(int n, int R1, int t) { const int nb = n / R1; const int j = t / nb; return pcell(R1 * (t - j * nb) + j); }
+
+template <int R, bool INV, class Cfg>
+__device__ __forceinline__ void line_first_smem(const LineCtx &c, const Cfg &cfg) {
+    const int nb = cfg.n() / R;
+#pragma unroll 1
+    for (int b = c.slot; b < nb; b += LINE_SLOTS) {
+        float2 v[R];
+        float2 *o = c.sm + pcell(R * b) * 4 + c.pl;
 #pragma unroll
-    for (int cc = 0; cc < MAXC; ++cc) {
-        const int b = c.bt + cc * c.nbt;
-        if (b < nb) {
-            float2 a0[R], a1[R], w[R];
+        for (int j = 0; j < R; ++j) v[j] = o[j * 4];
+        Bfly<R, INV>::run(v);
+        twiddle_mul<R, INV>(c.tw, b * cfg.tws(), v);
 #pragma unroll
-            for (int j = 0; j < R; ++j) { a0[j] = make_float2(v[cc][j].x, v[cc][j].y); a1[j] = make_float2(v[cc][j].z, v[cc][j].w); }
-            Bfly<R>::run(a0, c.dir); Bfly<R>::run(a1, c.dir);
-            line_twiddles<R>(c, b, w);
+        for (int k = 0; k < R; ++k) o[k * 4] = v[k];
+    }
+    __syncthreads();
+}
+
+// pass i (not the last): in place.  s = R1 .. R_{i-1}, ni = n / s.
+template <int R, bool INV, class Cfg>
+__device__ __forceinline__ void line_mid(const LineCtx &c, const Cfg &cfg, int s) {
+    const int n = cfg.n(), R1 = cfg.radix(0);
+    const int ni = n / s, sub = ni / R;                 // sub = n_i / R_i = range of b_i
+    const int ntask = n / R;
+    const bool fast = ((R1 * sub) & 15) == 0;
+    const int step = pcell(R1 * sub) * 4;
+#pragma unroll 1
+    for (int T = c.slot; T < ntask; T += LINE_SLOTS) {
+        const int k1 = T % R1, rest = T / R1;
+        const int outer = rest / sub, bi = rest - outer * sub;
+        const int c0 = R1 * (outer * ni + bi) + k1;
+        float2 v[R];
+        float2 *p0 = c.sm + pcell(c0) * 4 + c.pl;
+        if (fast) {
 #pragma unroll
-            for (int k = 0; k < R; ++k) {
-                const int o = pidx(R * b + k);
-                s0[o] = k ? cmul(a0[k], w[k]) : a0[k];
-                s1[o] = k ? cmul(a1[k], w[k]) : a1[k];
-            }
+            for (int j = 0; j < R; ++j) v[j] = p0[j * step];
+        } else {
+#pragma unroll
+            for (int j = 0; j < R; ++j) v[j] = c.sm[pcell(c0 + j * R1 * sub) * 4 + c.pl];
+        }
+        Bfly<R, INV>::run(v);
+        twiddle_mul<R, INV>(c.tw, bi * s * cfg.tws(), v);
+        if (fast) {
+#pragma unroll
+            for (int j = 0; j < R; ++j) p0[j * step] = v[j];
+        } else {
+#pragma unroll
+            for (int j = 0; j < R; ++j) c.sm[pcell(c0 + j * R1 * sub) * 4 + c.pl] = v[j];
         }
     }
     __syncthreads();
 }
 
-template <int R, int E>
-__device__ __forceinline__ void line_mid_pass(const LineCtx &c, int log2s) {
-    constexpr int MAXC = (E + R - 1) / R;
-    const int nb = c.n / R, s = 1 << log2s, m = nb >> log2s;
-    float2 *s0 = c.sm + (2 * c.pp) * c.ps, *s1 = s0 + c.ps;
-    float2 a0[MAXC][R], a1[MAXC][R];
+// last pass: shared -> global (through st).  Task T = k1 + R1 (k2 + R2 (k3 + ...)) < n / R, so that the R outputs
+// X[T + (n/R) k] of consecutive tasks are consecutive; the middle digits k2.. sit in shared memory in position
+// order (k2 most significant), hence the digit walk.
+template <int R, bool INV, class Cfg, class ST>
+__device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, ST st) {
+    const int n = cfg.n(), R1 = cfg.radix(0), ntask = n / R;
+    const bool fast = (R1 & 15) == 0;
+    const int step = pcell(R1) * 4;
+#pragma unroll 1
+    for (int T = c.slot; T < ntask; T += LINE_SLOTS) {
+        const int k1 = T % R1;
+        int rem = T / R1, mult = n / R1, B0 = 0;
 #pragma unroll
-    for (int cc = 0; cc < MAXC; ++cc) {
-        const int b = c.bt + cc * c.nbt;
-        if (b < nb) {
-            const int p = b >> log2s, q = b & (s - 1);
-#pragma unroll
-            for (int j = 0; j < R; ++j) {
-                const int o = pidx(q + ((p + m * j) << log2s));
-                a0[cc][j] = s0[o]; a1[cc][j] = s1[o];
-            }
+        for (int i = 1; i + 1 < cfg.npass(); ++i) {
+            const int Ri = cfg.radix(i);
+            mult /= Ri;
+            const int q = rem / Ri;
+            B0 += (rem - q * Ri) * mult;
+            rem = q;
         }
-    }
-    __syncthreads();
+        const int c0 = R1 * B0 + k1;
+        float2 v[R];
+        if (fast) {
+            const float2 *p0 = c.sm + pcell(c0) * 4 + c.pl;
 #pragma unroll
-    for (int cc = 0; cc < MAXC; ++cc) {
-        const int b = c.bt + cc * c.nbt;
-        if (b < nb) {
-            const int p = b >> log2s, q = b & (s - 1);
-            float2 w[R];
-            Bfly<R>::run(a0[cc], c.dir); Bfly<R>::run(a1[cc], c.dir);
-            line_twiddles<R>(c, p << log2s, w);
+            for (int j = 0; j < R; ++j) v[j] = p0[j * step];
+        } else {
 #pragma unroll
-            for (int k = 0; k < R; ++k) {
-                const int o = pidx(q + ((R * p + k) << log2s));
-                s0[o] = k ? cmul(a0[cc][k], w[k]) : a0[cc][k];
-                s1[o] = k ? cmul(a1[cc][k], w[k]) : a1[cc][k];
-            }
+            for (int j = 0; j < R; ++j) v[j] = c.sm[pcell(c0 + j * R1) * 4 + c.pl];
         }
-    }
-    __syncthreads();
-}
-
-template <int R, int E, class ST>
-__device__ __forceinline__ void line_last_pass(const LineCtx &c, ST st) {
-    constexpr int MAXC = (E + R - 1) / R;
-    const int s = c.n / R;                      // m = 1: p = 0, q = b
-    const float2 *s0 = c.sm + (2 * c.pp) * c.ps, *s1 = s0 + c.ps;
+        Bfly<R, INV>::run(v);
 #pragma unroll
-    for (int cc = 0; cc < MAXC; ++cc) {
-        const int b = c.bt + cc * c.nbt;
-        if (b < s) {
-            float2 a0[R], a1[R];
-#pragma unroll
-            for (int j = 0; j < R; ++j) { const int o = pidx(b + s * j); a0[j] = s0[o]; a1[j] = s1[o]; }
-            Bfly<R>::run(a0, c.dir); Bfly<R>::run(a1, c.dir);
-#pragma unroll
-            for (int k = 0; k < R; ++k) st(b + s * k, make_float4(a0[k].x, a0[k].y, a1[k].x, a1[k].y));
-        }
+        for (int k = 0; k < R; ++k) st(T + ntask * k, v[k]);
     }
 }
 
-__device__ __forceinline__ LineCtx line_ctx(float2 *sm, const FftDesc &d, const float2 *tw, float dir) {
+__device__ __forceinline__ LineCtx line_ctx(float2 *sm, const float2 *tw) {
     LineCtx c;
-    c.sm = sm; c.tw = tw; c.n = d.n; c.ps = d.ps; c.pp = threadIdx.x & 1; c.bt = threadIdx.x >> 1; c.nbt = blockDim.x >> 1; c.dir = dir;
+    c.sm = sm; c.tw = tw; c.pl = threadIdx.x & 3; c.slot = threadIdx.x >> 2;
     return c;
 }
 
-// Passes after the first: radix-8 passes from stride 2^ls, then the fused last pass (radix 8, or 5 if d.five).
-template <int E, class ST>
-__device__ __forceinline__ void line_finish(const LineCtx &c, const FftDesc &d, int ls, int n8_left, ST st) {
-    const int nmid = d.five ? n8_left : n8_left - 1;
+// ---- drivers: compile-time pass list ------------------------------------------------------------------
+template <bool INV, class Cfg, int I, int S_, class ST>
+__device__ __forceinline__ void static_finish(const LineCtx &c, const Cfg &cfg, ST st) {
+    constexpr int R = Cfg::radix(I);
+    if constexpr (I + 1 < Cfg::NP) {
+        line_mid<R, INV>(c, cfg, S_);
+        static_finish<INV, Cfg, I + 1, S_ * R>(c, cfg, st);
+    } else {
+        line_last<R, INV>(c, cfg, st);
+    }
+}
+
+// ---- drivers: run-time pass list ----------------------------------------------------------------------
+template <bool INV, class Cfg, class ST>
+__device__ __forceinline__ void runtime_finish(const LineCtx &c, const Cfg &cfg, ST st) {
+    int s = cfg.radix(0);
 #pragma unroll 1
-    for (int i = 0; i < nmid; ++i, ls += 3) line_mid_pass<8, E>(c, ls);
-    if (d.five) line_last_pass<5, E>(c, st);
-    else line_last_pass<8, E>(c, st);
+    for (int i = 1; i + 1 < cfg.npass(); ++i) {
+        const int R = cfg.radix(i);
+        if (R == 16) line_mid<16, INV>(c, cfg, s);
+        else if (R == 8) line_mid<8, INV>(c, cfg, s);
+        else if (R == 4) line_mid<4, INV>(c, cfg, s);
+        else line_mid<2, INV>(c, cfg, s);
+        s *= R;
+    }
+    const int RL = cfg.radix(cfg.npass() - 1);
+    if (RL == 16) line_last<16, INV>(c, cfg, st);
+    else if (RL == 8) line_last<8, INV>(c, cfg, st);
+    else if (RL == 5) line_last<5, INV>(c, cfg, st);
+    else if (RL == 4) line_last<4, INV>(c, cfg, st);
+    else line_last<2, INV>(c, cfg, st);
 }
 
-// global -> FFT -> global.  Needs at least two passes (n >= 16, not 2 or 4 alone).
-template <int E, class LD, class ST>
-__device__ __forceinline__ void fft_line(float2 *sm, const FftDesc &d, const float2 *tw, float dir, LD ld, ST st) {
-    const LineCtx c = line_ctx(sm, d, tw, dir);
-    if (d.first == 2) { line_first_pass<2, E>(c, ld); line_finish<E>(c, d, 1, d.n8, st); }
-    else if (d.first == 4) { line_first_pass<4, E>(c, ld); line_finish<E>(c, d, 2, d.n8, st); }
-    else { line_first_pass<8, E>(c, ld); line_finish<E>(c, d, 3, d.n8 - 1, st); }
+// global -> FFT -> global.  ld(t) returns this thread's plane of input element t; st(k, v) takes output k.
+// A barrier must separate two transforms that use the same shared memory (the caller's job).
+template <bool INV, class Cfg, class LD, class ST>
+__device__ __forceinline__ void fft_line(float2 *sm, const Cfg &cfg, const float2 *tw, LD ld, ST st) {
+    const LineCtx c = line_ctx(sm, tw);
+    if constexpr (Cfg::is_static) {
+        line_first<Cfg::radix(0), INV>(c, cfg, ld);
+        static_finish<INV, Cfg, 1, Cfg::radix(0)>(c, cfg, st);
+    } else {
+        const int R1 = cfg.radix(0);
+        if (R1 == 16) line_first<16, INV>(c, cfg, ld);
+        else if (R1 == 8) line_first<8, INV>(c, cfg, ld);
+        else if (R1 == 4) line_first<4, INV>(c, cfg, ld);
+        else line_first<2, INV>(c, cfg, ld);
+        runtime_finish<INV>(c, cfg, st);
+    }
 }
 
-// shared (already filled and synchronised) -> FFT -> global.
-template <int E, class ST>
-__device__ __forceinline__ void fft_line_from_smem(float2 *sm, const FftDesc &d, const float2 *tw, float dir, ST st) {
-    const LineCtx c = line_ctx(sm, d, tw, dir);
-    int ls = 0;
-    if (d.first == 2) { line_mid_pass<2, E>(c, 0); ls = 1; }
-    else if (d.first == 4) { line_mid_pass<4, E>(c, 0); ls = 2; }
-    line_finish<E>(c, d, ls, d.n8, st);
+// shared (filled at line_input_cell positions and synchronised by the caller) -> FFT -> global.
+template <bool INV, class Cfg, class ST>
+__device__ __forceinline__ void fft_line_from_smem(float2 *sm, const Cfg &cfg, const float2 *tw, ST st) {
+    const LineCtx c = line_ctx(sm, tw);
+    if constexpr (Cfg::is_static) {
+        line_first_smem<Cfg::radix(0), INV>(c, cfg);
+        static_finish<INV, Cfg, 1, Cfg::radix(0)>(c, cfg, st);
+    } else {
+        const int R1 = cfg.radix(0);
+        if (R1 == 16) line_first_smem<16, INV>(c, cfg);
+        else if (R1 == 8) line_first_smem<8, INV>(c, cfg);
+        else if (R1 == 4) line_first_smem<4, INV>(c, cfg);
+        else line_first_smem<2, INV>(c, cfg);
+        runtime_finish<INV>(c, cfg, st);
+    }
 }
 
 }  // namespace tc

@@ -21,85 +21,129 @@ extern __shared__ float4 smem_f4[];
 __device__ __forceinline__ int wrap(int i, int G) { return i < 0 ? i + G : (i >= G ? i - G : i); }
 
 // ------------------------------------------------------------------------------------------------
-// Line kernels: grid = (lines, groups); one CTA = one line of the 4 planes of a group; blockDim = 2 * slots
-// (see fft_line.cuh).  E = 8 for lengths <= 4096 (1024 threads, <= 64 registers), 16 above.
-#define TC_LB(E) __launch_bounds__((E) == 8 ? 1024 : 768)
+// Line kernels: grid = (lines, groups); one CTA of LINE_THREADS = one line of the 4 planes of a group (fft_line.cuh).
+//
+// Pruned split.  The fine grid has G = 2 n points per axis but only n of them carry data on the image side
+// (zero padding, eq. (8)), so a length-G transform with n non-zero inputs is two length-n transforms:
+//   Ghat[2 r + p] = sum_t h[t] mu_p(t) e^{-2 pi i r t / n},   p = 0, 1,   mu_p(t) = e^{-2 pi i p X(t) / G},
+// where t < n runs over the image samples in wrapped order (t < n/2: image index t + n/2, periodic fine-grid
+// index X = t; t >= n/2: image index t - n/2, X = t + n).  The adjoint direction is the transpose: two length-n
+// inverse transforms of the even and odd inputs, the second multiplied by conj(mu_1) and added to the first.
+// A line therefore needs n (not G) cells of shared memory and three CTAs fit on an SM, so one CTA's loads
+// overlap another's butterflies.
+// Layouts (cells of P = 4 planes = 32 bytes): a sector-wide (32-byte) column access runs at 4.4 TB/s for loads but
+// 2.8 TB/s for stores on B200 (measured), so every store stream below is contiguous and only two load streams
+// are strided:
+//   forward  rowbuf[g][i][x & 1][x >> 1]      rows written contiguously (F1), columns read with a row stride (F2)
+//   grid     grid[g][x][y & 1][y >> 1]        column-major: F2 writes and B3 reads whole columns contiguously; the
+//                                             polar kernels address single cells and do not care
+//   adjoint  rowbuf[g][x][i]                  columns written contiguously (B3), rows read with a column stride (B3 rows)
+#define TC_LB __launch_bounds__(LINE_THREADS, 2)
 
-// periodic index on the fine grid -> image index, or -1 in the zero padding
-__device__ __forceinline__ int unpad(int x, int n, int G) { return x < n / 2 ? x + n / 2 : (x >= G - n / 2 ? x - (G - n / 2) : -1); }
+template <class Cfg> __device__ __forceinline__ Cfg make_cfg(const FftDesc &f, int tws) {
+    if constexpr (Cfg::is_static) return Cfg{};
+    else return Cfg{f, tws};
+}
+
+struct Wrapped { int img, X; };      // image index and periodic fine-grid index of wrapped sample t
+__device__ __forceinline__ Wrapped wrapped(int t, int n) { const int h = n >> 1; Wrapped w; w.img = t < h ? t + h : t - h; w.X = t < h ? t : t + n; return w; }
 
 // F1 + row FFT.  eq. (8) read backwards: g = f d(y_i) d(x_j), zero-padded to G at periodic index.
-template <int E>
-__global__ void TC_LB(E) k_fwd_rows(DevPlan d, const float *__restrict__ vol, int S, float2 *__restrict__ rowbuf) {
+template <class Cfg>
+__global__ void TC_LB k_fwd_rows(DevPlan d, const float *__restrict__ vol, int S, float2 *__restrict__ rowbuf) {
     float2 *sm = reinterpret_cast<float2 *>(smem_f4);
-    const int i = blockIdx.x, g = blockIdx.y, n = d.n, G = d.G, pp = threadIdx.x & 1;
+    const Cfg cfg = make_cfg<Cfg>(d.fN, 2);
+    const int i = blockIdx.x, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = threadIdx.x & 3;
     const float di = d.deapod[i];
-    const int s0 = 8 * g + 4 * pp;                            // this thread's 4 slices: s0 .. s0+3
-    const float *v0 = vol + ((size_t)s0 * n + i) * n;
-    const size_t ss = (size_t)n * n;
-    float4 *out = reinterpret_cast<float4 *>(rowbuf) + ((size_t)g * n + i) * G * 2 + pp;
-    fft_line<E>(sm, d.fG, d.twG, -1.f,
-        [&](int x) {
-            const int j = unpad(x, n, G);
-            float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (j >= 0) {
-                const float w = di * d.deapod[j];
-                if (s0 < S) r.x = v0[j] * w;
-                if (s0 + 1 < S) r.y = v0[ss + j] * w;
-                if (s0 + 2 < S) r.z = v0[2 * ss + j] * w;
-                if (s0 + 3 < S) r.w = v0[3 * ss + j] * w;
-            }
-            return r;
-        },
-        [&](int x, float4 v) { out[(size_t)x * 2] = v; });
+    const int sre = 8 * g + 2 * pl;
+    const bool hre = sre < S, him = sre + 1 < S;
+    const float *vre = vol + ((size_t)sre * n + i) * n, *vim = vre + (size_t)n * n;
+    float2 *out = rowbuf + ((size_t)g * n + i) * G * 4 + pl;
+#pragma unroll 1
+    for (int p = 0; p < 2; ++p) {
+        fft_line<false>(sm, cfg, d.twG,
+            [&](int t) {
+                const Wrapped w = wrapped(t, n);
+                const float sc = di * __ldg(&d.deapod[w.img]);
+                float2 v = make_float2(hre ? __ldg(&vre[w.img]) * sc : 0.f, him ? __ldg(&vim[w.img]) * sc : 0.f);
+                if (p) v = cmul(v, __ldg(&d.twG[w.X]));
+                return v;
+            },
+            [&](int r, float2 v) { out[(size_t)(p * n + r) * 4] = v; });
+        __syncthreads();
+    }
 }
 
-// F2 column FFT; only the n non-zero rows are read.
-template <int E>
-__global__ void TC_LB(E) k_fwd_cols(DevPlan d, const float2 *__restrict__ rowbuf, float2 *__restrict__ grid) {
+// F2 column FFT; only the n non-zero rows exist in rowbuf.
+template <class Cfg>
+__global__ void TC_LB k_fwd_cols(DevPlan d, const float2 *__restrict__ rowbuf, float2 *__restrict__ grid) {
     float2 *sm = reinterpret_cast<float2 *>(smem_f4);
-    const int x = blockIdx.x, g = blockIdx.y, n = d.n, G = d.G, pp = threadIdx.x & 1;
-    const float4 *in = reinterpret_cast<const float4 *>(rowbuf) + ((size_t)g * n * G + x) * 2 + pp;
-    float4 *out = reinterpret_cast<float4 *>(grid) + ((size_t)g * G * G + x) * 2 + pp;
-    fft_line<E>(sm, d.fG, d.twG, -1.f,
-        [&](int y) { const int i = unpad(y, n, G); return i >= 0 ? __ldg(&in[(size_t)i * G * 2]) : make_float4(0.f, 0.f, 0.f, 0.f); },
-        [&](int y, float4 v) { out[(size_t)y * G * 2] = v; });
+    const Cfg cfg = make_cfg<Cfg>(d.fN, 2);
+    const int x = blockIdx.x, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = threadIdx.x & 3;
+    const float2 *in = rowbuf + ((size_t)g * n * G + (size_t)(x & 1) * n + (x >> 1)) * 4 + pl;
+    float2 *out = grid + ((size_t)g * G + x) * G * 4 + pl;
+#pragma unroll 1
+    for (int p = 0; p < 2; ++p) {
+        fft_line<false>(sm, cfg, d.twG,
+            [&](int t) {
+                const Wrapped w = wrapped(t, n);
+                float2 v = __ldg(&in[(size_t)w.img * G * 4]);
+                if (p) v = cmul(v, __ldg(&d.twG[w.X]));
+                return v;
+            },
+            [&](int r, float2 v) { out[(p * n + r) * 4] = v; });
+        __syncthreads();
+    }
 }
 
-// B3 inverse column FFT (unnormalised, eq. (8)); only the n rows of the crop are written.
-template <int E>
-__global__ void TC_LB(E) k_adj_cols(DevPlan d, const float2 *__restrict__ grid, float2 *__restrict__ rowbuf) {
+// B3 inverse column FFT (unnormalised, eq. (8)); only the n rows of the crop are produced.
+template <class Cfg>
+__global__ void TC_LB k_adj_cols(DevPlan d, const float2 *__restrict__ grid, float2 *rowbuf) {
     float2 *sm = reinterpret_cast<float2 *>(smem_f4);
-    const int x = blockIdx.x, g = blockIdx.y, n = d.n, G = d.G, pp = threadIdx.x & 1;
-    const float4 *in = reinterpret_cast<const float4 *>(grid) + ((size_t)g * G * G + x) * 2 + pp;
-    float4 *out = reinterpret_cast<float4 *>(rowbuf) + ((size_t)g * n * G + x) * 2 + pp;
-    fft_line<E>(sm, d.fG, d.twG, +1.f,
-        [&](int y) { return __ldg(&in[(size_t)y * G * 2]); },
-        [&](int y, float4 v) { const int i = unpad(y, n, G); if (i >= 0) out[(size_t)i * G * 2] = v; });
+    const Cfg cfg = make_cfg<Cfg>(d.fN, 2);
+    const int x = blockIdx.x, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = threadIdx.x & 3;
+    const float2 *in = grid + ((size_t)g * G + x) * G * 4 + pl;
+    float2 *out = rowbuf + ((size_t)g * G + x) * n * 4 + pl;                 // adjoint half-plane, column-major: [g][x][i]
+#pragma unroll 1
+    for (int p = 0; p < 2; ++p) {
+        fft_line<true>(sm, cfg, d.twG,
+            [&](int k) { return __ldg(&in[(p * n + k) * 4]); },
+            [&](int t, float2 v) {
+                const Wrapped w = wrapped(t, n);
+                float2 *o = out + w.img * 4;
+                if (p) { v = cmulc(v, __ldg(&d.twG[w.X])); v = cadd(v, *o); }     // this thread wrote *o in phase 0
+                *o = v;
+            });
+        __syncthreads();
+    }
 }
 
-// B3 inverse row FFT + B4 crop and deapodise ("division by phihat"); re -> slice 2p, im -> 2p+1.
-template <int E>
-__global__ void TC_LB(E) k_adj_rows(DevPlan d, const float2 *__restrict__ rowbuf, int S, float *__restrict__ vol) {
+// B3 inverse row FFT + B4 crop and deapodise ("division by phihat"); re -> slice 2 pl, im -> 2 pl + 1.
+template <class Cfg>
+__global__ void TC_LB k_adj_rows(DevPlan d, const float2 *__restrict__ rowbuf, int S, float *vol) {
     float2 *sm = reinterpret_cast<float2 *>(smem_f4);
-    const int i = blockIdx.x, g = blockIdx.y, n = d.n, G = d.G, pp = threadIdx.x & 1;
-    const float4 *in = reinterpret_cast<const float4 *>(rowbuf) + ((size_t)g * n + i) * G * 2 + pp;
+    const Cfg cfg = make_cfg<Cfg>(d.fN, 2);
+    const int i = blockIdx.x, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = threadIdx.x & 3;
+    const float2 *in = rowbuf + ((size_t)g * G * n + i) * 4 + pl;
     const float di = d.deapod[i];
-    const int s0 = 8 * g + 4 * pp;
-    float *v0 = vol + ((size_t)s0 * n + i) * n;
-    const size_t ss = (size_t)n * n;
-    fft_line<E>(sm, d.fG, d.twG, +1.f,
-        [&](int x) { return __ldg(&in[(size_t)x * 2]); },
-        [&](int x, float4 v) {
-            const int j = unpad(x, n, G);
-            if (j >= 0) {
-                const float w = di * d.deapod[j];
-                if (s0 < S) v0[j] = v.x * w;
-                if (s0 + 1 < S) v0[ss + j] = v.y * w;
-                if (s0 + 2 < S) v0[2 * ss + j] = v.z * w;
-                if (s0 + 3 < S) v0[3 * ss + j] = v.w * w;
-            }
-        });
+    const int sre = 8 * g + 2 * pl;
+    const bool hre = sre < S, him = sre + 1 < S;
+    float *vre = vol + ((size_t)sre * n + i) * n, *vim = vre + (size_t)n * n;
+#pragma unroll 1
+    for (int p = 0; p < 2; ++p) {
+        fft_line<true>(sm, cfg, d.twG,
+            [&](int k) { return __ldg(&in[(size_t)(2 * k + p) * n * 4]); },
+            [&](int t, float2 v) {
+                const Wrapped w = wrapped(t, n);
+                const float sc = di * __ldg(&d.deapod[w.img]);
+                if (p) v = cmulc(v, __ldg(&d.twG[w.X]));
+                v.x *= sc; v.y *= sc;
+                if (p) { if (hre) v.x += vre[w.img]; if (him) v.y += vim[w.img]; }  // this thread wrote them in phase 0
+                if (hre) vre[w.img] = v.x;
+                if (him) vim[w.img] = v.y;
+            });
+        __syncthreads();
+    }
 }
 
 #include "kernels_polar.inc"

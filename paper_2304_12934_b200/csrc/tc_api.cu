@@ -107,16 +107,23 @@ static void kb_poly(int W, double sigma, float *out) {
     }
 }
 
+// n = 2^a 5^b (b <= 1) as a pass list for the line engine: radix-16 passes first, then 8 / 4 / 2, the radix-5 pass last.
 static bool make_fft_desc(int n, FftDesc &f) {
     int m = n, fives = 0, twos = 0;
     while (m % 5 == 0) { m /= 5; ++fives; }
     while (m % 2 == 0) { m /= 2; ++twos; }
-    if (m != 1 || fives > 1 || (twos % 3 != 0) + twos / 3 + fives < 2) return false;   // at least two passes
-    f.n = n; f.ps = n + (n >> 4) + 1;
-    while (f.ps % 8 != 4) ++f.ps;                 // plane pairs of the two lanes of a thread pair land on complementary banks
-    f.first = twos % 3 == 1 ? 2 : (twos % 3 == 2 ? 4 : 0);
-    f.n8 = twos / 3; f.five = fives;
-    return true;
+    if (m != 1 || fives > 1) return false;
+    f.n = n; f.npass = 0;
+    while (twos >= 4) { f.radix[f.npass++] = 16; twos -= 4; if (f.npass >= FFT_MAX_PASSES - 1) break; }
+    if (twos >= 4) return false;
+    if (twos > 0) f.radix[f.npass++] = 1 << twos;
+    if (fives) f.radix[f.npass++] = 5;
+    if (f.npass < 2) {                              // 16 -> 4 x 4, 8 -> 4 x 2, 4 -> 2 x 2; 2 and 5 alone are not supported
+        if (f.npass == 1 && f.radix[0] >= 4) { const int r = f.radix[0]; f.radix[0] = r == 4 ? 2 : 4; f.radix[1] = r / f.radix[0]; f.npass = 2; }
+        else return false;
+    }
+    f.smem_cells = n + (n >> 4) + 1;
+    return (size_t)f.smem_cells * 32 <= 227 * 1024 - 1024;
 }
 
 template <typename T> static cudaError_t upload(T **dst, const std::vector<T> &h) {
@@ -142,7 +149,7 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
     const int n = gm->n, nd = gm->n_det, na = gm->n_angles, G = 2 * n;
     DevPlan &d = p->d;
     d.n = n; d.nd = nd; d.na = na; d.G = G; d.sc = (double)G / nd;
-    if (!make_fft_desc(G, d.fG) || !make_fft_desc(nd, d.fD)) { delete p; return fail(TC_EUNSUPPORTED, "2n and n_det must be 2^a 5^b, b <= 1, >= 8"); }
+    if (!make_fft_desc(n, d.fN) || !make_fft_desc(nd, d.fD)) { delete p; return fail(TC_EUNSUPPORTED, "n and n_det must be 2^a 5^b with b <= 1 (and at most 6800)"); }
     if (nd / 2 - 1 > 0 && d.sc * (nd / 2 - 1) + 3 >= G / 2 + 3) { /* taps wrap at most once; always true for sc = G/nd */ }
 
     const int W = KB_W; const double sigma = 2.0;
@@ -174,8 +181,9 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
     std::vector<int> order(na);
     std::vector<double> thm(na);
     for (int a = 0; a < na; ++a) {
-        const double th = (double)p->angles[a];
-        cs[a] = make_double2(d.sc * std::cos(th), d.sc * std::sin(th));
+        // the polar kernels work on the transposed (column-major) fine grid: swap the axes (exactly), theta' = pi/2 - theta
+        const double th = 0.5 * M_PI - (double)p->angles[a];
+        cs[a] = make_double2(d.sc * std::sin((double)p->angles[a]), d.sc * std::cos((double)p->angles[a]));
         double r = std::fmod(th, M_PI); if (r < 0) r += M_PI;
         thm[a] = r; order[a] = a;
     }
