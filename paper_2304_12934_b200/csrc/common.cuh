@@ -7,6 +7,7 @@ namespace tc {
 
 constexpr int KB_W = 6;          // Kaiser-Bessel window width (taps per axis)
 constexpr int KB_DEG = 12;       // degree of the window polynomial in z = 2 q - 1, q = 1 - (2 r / W)^2
+constexpr unsigned SPREAD_HEAVY = 32;   // tap lists longer than this are handled by one warp per cell (k_adj_spread_heavy)
 constexpr int P = 4;             // complex planes interleaved per fine-grid cell (= 8 real slices, 32 B)
 
 struct TileRange { int start, count, shx, shy; };   // angles (sorted order) whose ray can touch a 32 x 8 tile, per wrap alias
@@ -28,6 +29,8 @@ struct DevPlan {
     const int *tile_nr;           // [tiles] number of valid ranges
     const unsigned *tap_offs;     // [tiles * 256 + 1] CSR offsets of the spread's per-cell tap lists (cell order: tile, then thread)
     const int2 *taps;             // (a * nd + (m mod nd), float weight bits)
+    const unsigned *heavy;        // [n_heavy] cells (cidx) whose list is longer than SPREAD_HEAVY
+    unsigned n_heavy;
     int J;                        // radial modes to try on each side of the nearest one: floor(3 sqrt2 / sc + 1/2)
 };
 
@@ -47,6 +50,7 @@ void launch_adj_radial(const DevPlan &d, const float *sino, int S, int ng, float
 void launch_tile_ranges(const DevPlan &d, TileRange *rng, int *nrng, cudaStream_t st);
 void launch_spread_count(const DevPlan &d, int *counts, cudaStream_t st);
 void launch_spread_fill(const DevPlan &d, cudaStream_t st);
+void launch_spread_heavy_list(const DevPlan &d, unsigned ncell, unsigned *list, unsigned *count, cudaStream_t st);
 void launch_adj_spread(const DevPlan &d, const float2 *cpol, int ng, float2 *grid, cudaStream_t st);
 // grid -> rowbuf (cropped to n rows)             (B3 inverse column FFT)
 void launch_adj_cols(const DevPlan &d, const float2 *grid, int ng, float2 *rowbuf, cudaStream_t st);

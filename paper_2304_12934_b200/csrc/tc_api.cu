@@ -41,6 +41,7 @@ struct tc_plan {
     TileRange *tile_rng = nullptr;
     unsigned *tap_offs = nullptr;
     int2 *taps = nullptr;
+    unsigned *heavy = nullptr;
     long long n_taps = 0;
     // scratch
     int ng_alloc = 0;
@@ -234,6 +235,17 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
         p->n_taps = total;
         d.tap_offs = p->tap_offs; d.taps = p->taps;
         launch_spread_fill(d, nullptr);
+        {   // cells with long lists: at most the disc of radius ~ 36 na / (2 pi SPREAD_HEAVY) cells; size the list for all cells with > SPREAD_HEAVY taps
+            const size_t cap = std::min<size_t>(nc, (size_t)total / SPREAD_HEAVY + 1);
+            unsigned *cnt = nullptr;
+            e = cudaMalloc((void **)&p->heavy, cap * sizeof(unsigned));
+            if (e == cudaSuccess) e = cudaMalloc((void **)&cnt, sizeof(unsigned));
+            if (e == cudaSuccess) e = cudaMemset(cnt, 0, sizeof(unsigned));
+            if (e == cudaSuccess) { launch_spread_heavy_list(d, (unsigned)nc, p->heavy, cnt, nullptr); e = cudaMemcpy(&d.n_heavy, cnt, sizeof(unsigned), cudaMemcpyDeviceToHost); }
+            cudaFree(cnt);
+            d.heavy = p->heavy;
+            if (e != cudaSuccess) { tc_plan_destroy(p); return fail(TC_ECUDA, std::string("spread heavy list: ") + cudaGetErrorString(e)); }
+        }
         e = cudaDeviceSynchronize();
         if (e != cudaSuccess) { tc_plan_destroy(p); return fail(TC_ECUDA, std::string("spread tap lists: ") + cudaGetErrorString(e)); }
     }
@@ -252,7 +264,7 @@ extern "C" tc_status tc_plan_destroy(tc_plan *p) {
     if (!p) return TC_OK;
     free_scratch(p);
     cudaFree(p->twG); cudaFree(p->twD); cudaFree(p->ph_fwd); cudaFree(p->ph_adj); cudaFree(p->deapod);
-    cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc); cudaFree(p->tile_rng); cudaFree(p->tile_nr); cudaFree(p->tap_offs); cudaFree(p->taps);
+    cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc); cudaFree(p->tile_rng); cudaFree(p->tile_nr); cudaFree(p->tap_offs); cudaFree(p->taps); cudaFree(p->heavy);
     if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
     if (p->s_comp) cudaStreamDestroy(p->s_comp);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
