@@ -83,7 +83,7 @@ __device__ __forceinline__ void line_first(const LineCtx &c, const Cfg &cfg, LD 
     for (int b = c.slot; b < nb; b += LINE_SLOTS) {
         float2 v[R];
 #pragma unroll
-        for (int j = 0; j < R; ++j) v[j] = ld(b + nb * j);
+        for (int j = 0; j < R; ++j) v[j] = ld(b + nb * j, R % 2 == 0 ? j < R / 2 : 2 * (b + nb * j) < cfg.n());
         Bfly<R, INV>::run(v);
         twiddle_mul<R, INV>(c.tw, b * cfg.tws(), v);
         float2 *o = c.sm + pcell(R * b) * 4 + c.pl;   // R b is a multiple of R and R divides 16: k never crosses a padding cell
@@ -152,8 +152,12 @@ __device__ __forceinline__ void line_mid(const LineCtx &c, const Cfg &cfg, int s
 // last pass: shared -> global (through st).  Task T = k1 + R1 (k2 + R2 (k3 + ...)) < n / R, so that the R outputs
 // X[T + (n/R) k] of consecutive tasks are consecutive; the middle digits k2.. sit in shared memory in position
 // order (k2 most significant), hence the digit walk.
-template <int R, bool INV, class Cfg, class ST>
-__device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, ST st) {
+// pre(k, lo) is called for the task's R outputs before the butterfly (a read-modify-write caller starts its loads
+// there) and its value is handed to st(k, lo, v, old).  lo = "k < n / 2", a compile-time fact for even radices.
+struct NoPre { __device__ __forceinline__ float2 operator()(int, bool) const { return make_float2(0.f, 0.f); } };
+
+template <int R, bool INV, class Cfg, class PRE, class ST>
+__device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, PRE pre, ST st) {
     const int n = cfg.n(), R1 = cfg.radix(0), ntask = n / R;
     const bool fast = (R1 & 15) == 0;
     const int step = pcell(R1) * 4;
@@ -170,7 +174,9 @@ __device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, ST s
             rem = q;
         }
         const int c0 = R1 * B0 + k1;
-        float2 v[R];
+        float2 v[R], old[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) old[k] = pre(T + ntask * k, R % 2 == 0 ? k < R / 2 : 2 * (T + ntask * k) < n);
         if (fast) {
             const float2 *p0 = c.sm + pcell(c0) * 4 + c.pl;
 #pragma unroll
@@ -181,7 +187,7 @@ __device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, ST s
         }
         Bfly<R, INV>::run(v);
 #pragma unroll
-        for (int k = 0; k < R; ++k) st(T + ntask * k, v[k]);
+        for (int k = 0; k < R; ++k) st(T + ntask * k, R % 2 == 0 ? k < R / 2 : 2 * (T + ntask * k) < n, v[k], old[k]);
     }
 }
 
@@ -192,20 +198,20 @@ __device__ __forceinline__ LineCtx line_ctx(float2 *sm, const float2 *tw) {
 }
 
 // ---- drivers: compile-time pass list ------------------------------------------------------------------
-template <bool INV, class Cfg, int I, int S_, class ST>
-__device__ __forceinline__ void static_finish(const LineCtx &c, const Cfg &cfg, ST st) {
+template <bool INV, class Cfg, int I, int S_, class PRE, class ST>
+__device__ __forceinline__ void static_finish(const LineCtx &c, const Cfg &cfg, PRE pre, ST st) {
     constexpr int R = Cfg::radix(I);
     if constexpr (I + 1 < Cfg::NP) {
         line_mid<R, INV>(c, cfg, S_);
-        static_finish<INV, Cfg, I + 1, S_ * R>(c, cfg, st);
+        static_finish<INV, Cfg, I + 1, S_ * R>(c, cfg, pre, st);
     } else {
-        line_last<R, INV>(c, cfg, st);
+        line_last<R, INV>(c, cfg, pre, st);
     }
 }
 
 // ---- drivers: run-time pass list ----------------------------------------------------------------------
-template <bool INV, class Cfg, class ST>
-__device__ __forceinline__ void runtime_finish(const LineCtx &c, const Cfg &cfg, ST st) {
+template <bool INV, class Cfg, class PRE, class ST>
+__device__ __forceinline__ void runtime_finish(const LineCtx &c, const Cfg &cfg, PRE pre, ST st) {
     int s = cfg.radix(0);
 #pragma unroll 1
     for (int i = 1; i + 1 < cfg.npass(); ++i) {
@@ -217,28 +223,28 @@ __device__ __forceinline__ void runtime_finish(const LineCtx &c, const Cfg &cfg,
         s *= R;
     }
     const int RL = cfg.radix(cfg.npass() - 1);
-    if (RL == 16) line_last<16, INV>(c, cfg, st);
-    else if (RL == 8) line_last<8, INV>(c, cfg, st);
-    else if (RL == 5) line_last<5, INV>(c, cfg, st);
-    else if (RL == 4) line_last<4, INV>(c, cfg, st);
-    else line_last<2, INV>(c, cfg, st);
+    if (RL == 16) line_last<16, INV>(c, cfg, pre, st);
+    else if (RL == 8) line_last<8, INV>(c, cfg, pre, st);
+    else if (RL == 5) line_last<5, INV>(c, cfg, pre, st);
+    else if (RL == 4) line_last<4, INV>(c, cfg, pre, st);
+    else line_last<2, INV>(c, cfg, pre, st);
 }
 
-// global -> FFT -> global.  ld(t) returns this thread's plane of input element t; st(k, v) takes output k.
+// global -> FFT -> global.  ld(t, lo) returns this thread's plane of input element t; st(k, lo, v, old) takes output k.
 // A barrier must separate two transforms that use the same shared memory (the caller's job).
-template <bool INV, class Cfg, class LD, class ST>
-__device__ __forceinline__ void fft_line(float2 *sm, const Cfg &cfg, const float2 *tw, LD ld, ST st) {
+template <bool INV, class Cfg, class LD, class PRE, class ST>
+__device__ __forceinline__ void fft_line(float2 *sm, const Cfg &cfg, const float2 *tw, LD ld, PRE pre, ST st) {
     const LineCtx c = line_ctx(sm, tw);
     if constexpr (Cfg::is_static) {
         line_first<Cfg::radix(0), INV>(c, cfg, ld);
-        static_finish<INV, Cfg, 1, Cfg::radix(0)>(c, cfg, st);
+        static_finish<INV, Cfg, 1, Cfg::radix(0)>(c, cfg, pre, st);
     } else {
         const int R1 = cfg.radix(0);
         if (R1 == 16) line_first<16, INV>(c, cfg, ld);
         else if (R1 == 8) line_first<8, INV>(c, cfg, ld);
         else if (R1 == 4) line_first<4, INV>(c, cfg, ld);
         else line_first<2, INV>(c, cfg, ld);
-        runtime_finish<INV>(c, cfg, st);
+        runtime_finish<INV>(c, cfg, pre, st);
     }
 }
 
@@ -248,14 +254,14 @@ __device__ __forceinline__ void fft_line_from_smem(float2 *sm, const Cfg &cfg, c
     const LineCtx c = line_ctx(sm, tw);
     if constexpr (Cfg::is_static) {
         line_first_smem<Cfg::radix(0), INV>(c, cfg);
-        static_finish<INV, Cfg, 1, Cfg::radix(0)>(c, cfg, st);
+        static_finish<INV, Cfg, 1, Cfg::radix(0)>(c, cfg, NoPre(), st);
     } else {
         const int R1 = cfg.radix(0);
         if (R1 == 16) line_first_smem<16, INV>(c, cfg);
         else if (R1 == 8) line_first_smem<8, INV>(c, cfg);
         else if (R1 == 4) line_first_smem<4, INV>(c, cfg);
         else line_first_smem<2, INV>(c, cfg);
-        runtime_finish<INV>(c, cfg, st);
+        runtime_finish<INV>(c, cfg, NoPre(), st);
     }
 }
 

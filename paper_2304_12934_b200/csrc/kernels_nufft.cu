@@ -45,8 +45,8 @@ template <class Cfg> __device__ __forceinline__ Cfg make_cfg(const FftDesc &f, i
     else return Cfg{f, tws};
 }
 
-struct Wrapped { int img, X; };      // image index and periodic fine-grid index of wrapped sample t
-__device__ __forceinline__ Wrapped wrapped(int t, int n) { const int h = n >> 1; Wrapped w; w.img = t < h ? t + h : t - h; w.X = t < h ? t : t + n; return w; }
+struct Wrapped { int img, X; };      // image index and periodic fine-grid index of wrapped sample t (lo = t < n / 2)
+__device__ __forceinline__ Wrapped wrapped(int t, int n, bool lo) { const int h = n >> 1; Wrapped w; w.img = lo ? t + h : t - h; w.X = lo ? t : t + n; return w; }
 
 // F1 + row FFT.  eq. (8) read backwards: g = f d(y_i) d(x_j), zero-padded to G at periodic index.
 template <class Cfg>
@@ -62,14 +62,14 @@ __global__ void TC_LB k_fwd_rows(DevPlan d, const float *__restrict__ vol, int S
 #pragma unroll 1
     for (int p = 0; p < 2; ++p) {
         fft_line<false>(sm, cfg, d.twG,
-            [&](int t) {
-                const Wrapped w = wrapped(t, n);
+            [&](int t, bool lo) {
+                const Wrapped w = wrapped(t, n, lo);
                 const float sc = di * __ldg(&d.deapod[w.img]);
                 float2 v = make_float2(hre ? __ldg(&vre[w.img]) * sc : 0.f, him ? __ldg(&vim[w.img]) * sc : 0.f);
                 if (p) v = cmul(v, __ldg(&d.twG[w.X]));
                 return v;
             },
-            [&](int r, float2 v) { out[(size_t)(p * n + r) * 4] = v; });
+            NoPre(), [&](int r, bool, float2 v, float2) { out[(size_t)(p * n + r) * 4] = v; });
         __syncthreads();
     }
 }
@@ -85,13 +85,13 @@ __global__ void TC_LB k_fwd_cols(DevPlan d, const float2 *__restrict__ rowbuf, f
 #pragma unroll 1
     for (int p = 0; p < 2; ++p) {
         fft_line<false>(sm, cfg, d.twG,
-            [&](int t) {
-                const Wrapped w = wrapped(t, n);
+            [&](int t, bool lo) {
+                const Wrapped w = wrapped(t, n, lo);
                 float2 v = __ldg(&in[(size_t)w.img * G * 4]);
                 if (p) v = cmul(v, __ldg(&d.twG[w.X]));
                 return v;
             },
-            [&](int r, float2 v) { out[(p * n + r) * 4] = v; });
+            NoPre(), [&](int r, bool, float2 v, float2) { out[(p * n + r) * 4] = v; });
         __syncthreads();
     }
 }
@@ -107,12 +107,12 @@ __global__ void TC_LB k_adj_cols(DevPlan d, const float2 *__restrict__ grid, flo
 #pragma unroll 1
     for (int p = 0; p < 2; ++p) {
         fft_line<true>(sm, cfg, d.twG,
-            [&](int k) { return __ldg(&in[(p * n + k) * 4]); },
-            [&](int t, float2 v) {
-                const Wrapped w = wrapped(t, n);
-                float2 *o = out + w.img * 4;
-                if (p) { v = cmulc(v, __ldg(&d.twG[w.X])); v = cadd(v, *o); }     // this thread wrote *o in phase 0
-                *o = v;
+            [&](int k, bool) { return __ldg(&in[(p * n + k) * 4]); },
+            [&](int t, bool lo) { return p ? out[wrapped(t, n, lo).img * 4] : make_float2(0.f, 0.f); },   // this thread wrote it in phase 0
+            [&](int t, bool lo, float2 v, float2 old) {
+                const Wrapped w = wrapped(t, n, lo);
+                if (p) { v = cmulc(v, __ldg(&d.twG[w.X])); v = cadd(v, old); }
+                out[w.img * 4] = v;
             });
         __syncthreads();
     }
@@ -132,13 +132,16 @@ __global__ void TC_LB k_adj_rows(DevPlan d, const float2 *__restrict__ rowbuf, i
 #pragma unroll 1
     for (int p = 0; p < 2; ++p) {
         fft_line<true>(sm, cfg, d.twG,
-            [&](int k) { return __ldg(&in[(size_t)(2 * k + p) * n * 4]); },
-            [&](int t, float2 v) {
-                const Wrapped w = wrapped(t, n);
+            [&](int k, bool) { return __ldg(&in[(size_t)(2 * k + p) * n * 4]); },
+            [&](int t, bool lo) {                                                   // this thread wrote them in phase 0
+                const int j = wrapped(t, n, lo).img;
+                return p ? make_float2(hre ? vre[j] : 0.f, him ? vim[j] : 0.f) : make_float2(0.f, 0.f);
+            },
+            [&](int t, bool lo, float2 v, float2 old) {
+                const Wrapped w = wrapped(t, n, lo);
                 const float sc = di * __ldg(&d.deapod[w.img]);
                 if (p) v = cmulc(v, __ldg(&d.twG[w.X]));
-                v.x *= sc; v.y *= sc;
-                if (p) { if (hre) v.x += vre[w.img]; if (him) v.y += vim[w.img]; }  // this thread wrote them in phase 0
+                v.x = fmaf(v.x, sc, old.x); v.y = fmaf(v.y, sc, old.y);
                 if (hre) vre[w.img] = v.x;
                 if (him) vim[w.img] = v.y;
             });
