@@ -64,11 +64,14 @@ void launch_extrapolate(const float *x, const float *xm, float beta, float *y, s
 // r = Ax + beta (Ax - Axm) - b ; Ay kept          (M1, sinogram part)
 void launch_residual(const float *Ax, const float *Axm, const float *b, float beta, float *Ay, float *r, size_t n, cudaStream_t st);
 // g = atr + lambda grad H(y);  z = y - g / L      (M2 + M3).  y has S slices of n x n; g may alias atr.
-void launch_update(const float *y, const float *atr, PriorDev pr, float invL, float *g, float *z, int S, int n, cudaStream_t st);
+// y has S slices; outputs are written for slices [s_first, s_first + n_out) only (n_out < 0: to the end) -- slabs with halos
+void launch_update(const float *y, const float *atr, PriorDev pr, float invL, float *g, float *z, int S, int n, cudaStream_t st,
+                   int s_first = 0, int n_out = -1);
 // Az = Ay - Ag / L;  acc[0] += 1/2 ||Az - b||^2   (M4 data term, fp64 accumulation)
 void launch_candidate_sino(const float *Ay, const float *Ag, const float *b, float invL, float *Az, double *acc, size_t n, cudaStream_t st);
 // acc[1] += H(z) over unordered 26-neighbour pairs (M4 prior term); grad (nullable) = grad H(z)
-void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, int n, cudaStream_t st);
+// pairs are owned by their lower slice; only owners among the first S_own slices are summed (S_own < 0: all)
+void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, int n, cudaStream_t st, int S_own = -1);
 // acc[slot] += sum v^2
 void launch_sumsq(const float *v, size_t n, double *acc, int slot, cudaStream_t st);
 void launch_scale(float *v, float a, size_t n, cudaStream_t st);

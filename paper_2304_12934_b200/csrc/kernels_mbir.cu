@@ -109,10 +109,10 @@ __device__ __forceinline__ float wgt(int dz, int dy, int dx) {
 // and its one-voxel halo for the three z-planes are staged in shared memory.
 template <bool STEP>
 __global__ void __launch_bounds__(256) k_prior_grad(const float *__restrict__ y, const float *atr, PriorK pk, float lambda,
-                                                     float invL, float *g, float *__restrict__ z, int S, int n) {
+                                                     float invL, float *g, float *__restrict__ z, int S, int n, int s_first) {
     __shared__ float t[3][10][34];
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 8, s = blockIdx.z;
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 8, s = blockIdx.z + s_first;
     for (int e = threadIdx.x; e < 3 * 10 * 34; e += 256) {
         const int dz = e / 340, r = e % 340, yy = r / 34, xx = r % 34;
         const int gz = s + dz - 1, gy = y0 + yy - 1, gx = x0 + xx - 1;
@@ -141,8 +141,8 @@ __global__ void __launch_bounds__(256) k_prior_grad(const float *__restrict__ y,
 }
 
 // M4 prior term: H(z) = sum over unordered pairs, each counted once through its 13 "forward" offsets.
-__global__ void __launch_bounds__(256) k_prior_value(const float *__restrict__ zv, PriorK pk, double *partials, int S, int n) {
-    const size_t total = (size_t)S * n * n;
+__global__ void __launch_bounds__(256) k_prior_value(const float *__restrict__ zv, PriorK pk, double *partials, int S, int n, int S_own) {
+    const size_t total = (size_t)S_own * n * n;      // pairs are owned by their lower slice; owners: the first S_own slices
     double sum = 0.0;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const int x = (int)(i % n), yy = (int)((i / n) % n), s = (int)(i / ((size_t)n * n));
@@ -174,20 +174,23 @@ void launch_extrapolate(const float *x, const float *xm, float beta, float *y, s
 void launch_residual(const float *Ax, const float *Axm, const float *b, float beta, float *Ay, float *r, size_t n, cudaStream_t st) {
     k_residual<<<ew_blocks(n), 256, 0, st>>>(Ax, Axm, b, beta, Ay, r, n); TC_COUNT_LAUNCH();
 }
-void launch_update(const float *y, const float *atr, PriorDev pr, float invL, float *g, float *z, int S, int n, cudaStream_t st) {
-    dim3 gr((n + 31) / 32, (n + 7) / 8, S);
-    if (z) k_prior_grad<true><<<gr, 256, 0, st>>>(y, atr, mk(pr), pr.lambda, invL, g, z, S, n);
-    else   k_prior_grad<false><<<gr, 256, 0, st>>>(y, atr, mk(pr), pr.lambda, invL, g, nullptr, S, n);
+void launch_update(const float *y, const float *atr, PriorDev pr, float invL, float *g, float *z, int S, int n, cudaStream_t st,
+                   int s_first, int n_out) {
+    if (n_out < 0) n_out = S - s_first;
+    dim3 gr((n + 31) / 32, (n + 7) / 8, n_out);
+    if (z) k_prior_grad<true><<<gr, 256, 0, st>>>(y, atr, mk(pr), pr.lambda, invL, g, z, S, n, s_first);
+    else   k_prior_grad<false><<<gr, 256, 0, st>>>(y, atr, mk(pr), pr.lambda, invL, g, nullptr, S, n, s_first);
     TC_COUNT_LAUNCH();
 }
 void launch_candidate_sino(const float *Ay, const float *Ag, const float *b, float invL, float *Az, double *acc, size_t n, cudaStream_t st) {
     k_candidate_sino<<<RED_BLOCKS, RED_THREADS, 0, st>>>(Ay, Ag, b, invL, Az, acc + 16, n); TC_COUNT_LAUNCH();
     final_reduce(acc, 0, 0.5, st);
 }
-void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, int n, cudaStream_t st) {
+void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, int n, cudaStream_t st, int S_own) {
+    if (S_own < 0) S_own = S;
     if (grad) { PriorDev p1 = pr; p1.lambda = 1.f; launch_update(z, nullptr, p1, 0.f, grad, nullptr, S, n, st); }
     if (acc) {
-        k_prior_value<<<RED_BLOCKS, RED_THREADS, 0, st>>>(z, mk(pr), acc + 16, S, n); TC_COUNT_LAUNCH();
+        k_prior_value<<<RED_BLOCKS, RED_THREADS, 0, st>>>(z, mk(pr), acc + 16, S, n, S_own); TC_COUNT_LAUNCH();
         final_reduce(acc, 1, 1.0, st);
     }
 }

@@ -349,4 +349,5 @@ static bool is_device_ptr(const void *ptr) {
     return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
 }
 
+#include "tc_api_part3.inc"
 #include "tc_api_part2.inc"

@@ -234,3 +234,33 @@ def test_full_size_config4_geometry_sampled(tc):
     plan = tc.Plan(c["N"], c["Nd"], ang, c["centre"])
     br = _np(plan.backproject(_cuda(yr))); plan.close()
     assert _adj_mismatch(vol, yr, s, br) < TOL_ADJ
+
+
+def test_mbir_out_of_core_streaming_matches_in_core_and_oracle(tc):
+    # S1 + M1-M5: host-resident sinogram and volume, slab size forced to 8 slices -> 3 slabs (8, 8, 3) with z-halos;
+    # the 26-neighbour prior couples the slabs, so a wrong halo shows up in both the iterate and F
+    from paper_2304_12934_b200 import inputs
+    from oracle import nufft, mbir
+    S, n, na = 19, 64, 24
+    ang = inputs.angles_uniform(na); a64 = ang.astype(np.float64)
+    vol = inputs.volume_cfg2(S=S, n=n)
+    b = (nufft.radon_nufft(vol, a64, n, 32.0) + 0.01 * np.random.default_rng(18).standard_normal((S, na, n))).astype(np.float32)
+    L, _ = mbir.lipschitz(n, a64, n, 32.0, P, SIG, C, 1.0)
+    pr = tc.prior_params(P, SIG, C, 1.0, L)
+    plan = tc.Plan(n, n, ang, 32.0)
+    x_in, log_in = plan.mbir(b, pr, 6)                                        # host pointers, fits: in-core
+    assert plan.sched_stats()["n_slabs"] == 0
+    plan.close()
+    plan = tc.Plan(n, n, ang, 32.0, max_slab_slices=8)
+    x_st, log_st = plan.mbir(b, pr, 6)                                        # forced streaming
+    st = plan.sched_stats()
+    plan.close()
+    assert st["n_slabs"] == 3 and st["h2d_bytes"] > 0 and st["d2h_bytes"] == 6 * (x_st.nbytes + b.nbytes)
+    assert rel_l2(x_st, x_in) <= 1e-6
+    assert [l["accepted"] for l in log_st] == [l["accepted"] for l in log_in]
+    for ls, li in zip(log_st, log_in):
+        assert abs(ls["F"] - li["F"]) <= 1e-9 * abs(li["F"])
+    xo, logo = mbir.mbir(b, a64, n, 32.0, P, SIG, C, 1.0, L, 6)
+    assert rel_l2(x_st, xo) < TOL_MBIR
+    F = [l["F"] for l in log_st]
+    assert all(F[i + 1] <= F[i] for i in range(len(F) - 1))
