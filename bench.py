@@ -26,6 +26,9 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--mbir", action="store_true", help="also time one MBIR iteration (extra.mbir_*)")
+    ap.add_argument("--ooc", type=int, default=0, metavar="SLICES",
+                    help="also run config 5's geometry (2560^2, 1313 angles) out of core on SLICES host-resident slices: "
+                         "streamed MBIR iterations, transfer/compute overlap (extra.ooc)")
     return ap.parse_args()
 
 
@@ -239,6 +242,31 @@ def main():
         extra["mbir_iter_ms"] = 1e3 * (t4 - t1) / 3
         extra["mbir_pairs_per_s"] = Sm * Na / ((t4 - t1) / 3)
         extra["mbir_slices"] = Sm
+
+    if args.ooc and rank == 0:
+        c5 = inputs.CONFIGS[5]
+        S5, N5, Na5 = args.ooc, c5["N"], c5["Na"]
+        plan.close()
+        del vol, sino, back
+        torch.cuda.empty_cache()
+        p5 = tc.Plan(N5, c5["Nd"], inputs.angles_uniform(Na5), c5["centre"], max_slab_slices=32)
+        v5 = torch.from_numpy(inputs.volume_fibres(S5, N5, c5["seed"], n_fibres=3000, workers=nw)).pin_memory()
+        b5 = torch.empty((S5, Na5, c5["Nd"]), dtype=torch.float32).pin_memory()
+        p5.radon(v5, out=b5)                                      # b = A truth, by the GPU path itself, slab-wise
+        st_f = p5.sched_stats()
+        pr5 = tc.prior_params(L=float(1.05 * 1.02 * Na5 * N5 + 4.0 / (1e-4 * (1 / 0.7) ** 2)))
+        its = 3
+        x5, log5 = p5.mbir(b5, pr5, its, out=torch.empty((S5, N5, N5), dtype=torch.float32).pin_memory())
+        st5 = p5.sched_stats()
+        extra["ooc"] = {"workload": "config5 geometry (2560x2560, 1313 angles, 2560 bins), %d of 2160 slices host-resident (pinned), slabs of 32, %d MBIR iterations" % (S5, its),
+                        "mbir_iter_s": st5["wall_s"] / its, "mbir_pairs_per_s": S5 * Na5 / (st5["wall_s"] / its),
+                        "overlap": st5["overlap"], "h2d_s": st5["h2d_s"], "compute_s": st5["compute_s"], "d2h_s": st5["d2h_s"], "wall_s": st5["wall_s"],
+                        "h2d_GBps": st5["h2d_bytes"] / max(st5["h2d_s"], 1e-9) / 1e9, "d2h_GBps": st5["d2h_bytes"] / max(st5["d2h_s"], 1e-9) / 1e9,
+                        "pcie_bytes_per_iter": (st5["h2d_bytes"] + st5["d2h_bytes"]) / its,
+                        "F": [l["F"] for l in log5], "accepted": [l["accepted"] for l in log5],
+                        "radon_streamed": {"wall_s": st_f["wall_s"], "overlap": st_f["overlap"], "pairs_per_s": S5 * Na5 / st_f["wall_s"]}}
+        p5.close()
+        plan = tc.Plan(N, Nd, ang, c["centre"])
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
