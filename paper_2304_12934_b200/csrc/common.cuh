@@ -7,7 +7,7 @@ namespace tc {
 
 constexpr int KB_W = 6;          // Kaiser-Bessel window width (taps per axis)
 constexpr int KB_DEG = 12;       // degree of the window polynomial in z = 2 q - 1, q = 1 - (2 r / W)^2
-constexpr unsigned SPREAD_HEAVY = 32;   // tap lists longer than this are handled by one warp per cell (k_adj_spread_heavy)
+constexpr unsigned SPREAD_HEAVY = 96;   // tap lists longer than this are handled by one warp per cell (k_adj_spread_heavy)
 constexpr int P = 4;             // complex planes interleaved per fine-grid cell (= 8 real slices, 32 B)
 
 struct TileRange { int start, count, shx, shy; };   // angles (sorted order) whose ray can touch a 32 x 8 tile, per wrap alias
