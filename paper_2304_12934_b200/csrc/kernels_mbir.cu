@@ -82,18 +82,22 @@ __global__ void k_scale(float *v, float a, size_t n) {
 // h(D) = u^2 / (c + u^(2-p)), h'(D) = sign(D)/sigma * u (2c + p u^(2-p)) / (c + u^(2-p))^2, u = |D|/sigma.
 struct PriorK { float inv_sigma, c, p, q; };     // q = 2 - p
 
-__device__ __forceinline__ float upow(float u, float q) { return exp2f(q * __log2f(u)); }   // u >= 0; 0 -> 0
+__device__ __forceinline__ float upow(float u, float q) {                                       // u >= 0; 0 -> 0 (lg2 -> -inf, ex2 -> 0)
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(q * __log2f(u)));
+    return r;
+}
 
 __device__ __forceinline__ float dh(float D, const PriorK &k) {
     const float u = fabsf(D) * k.inv_sigma;
     const float uq = upow(u, k.q);
     const float den = k.c + uq;
-    const float v = k.inv_sigma * u * fmaf(k.p, uq, 2.f * k.c) / (den * den);
+    const float v = __fdividef(k.inv_sigma * u * fmaf(k.p, uq, 2.f * k.c), den * den);     // MUFU.RCP + FMUL, 2 ulp
     return copysignf(v, D);
 }
 __device__ __forceinline__ float hval(float D, const PriorK &k) {
     const float u = fabsf(D) * k.inv_sigma;
-    return u * u / (k.c + upow(u, k.q));
+    return __fdividef(u * u, k.c + upow(u, k.q));
 }
 
 // w_mn = (1/dist) / (6 + 12/sqrt2 + 8/sqrt3)  (reading G10)
@@ -140,28 +144,51 @@ __global__ void __launch_bounds__(256) k_prior_grad(const float *__restrict__ y,
     if (STEP) z[o] = fmaf(-invL, gv, c0);
 }
 
-// M4 prior term: H(z) = sum over unordered pairs, each counted once through its 13 "forward" offsets.
+// M4 prior term: H(z) = sum over unordered pairs, each counted once through its 13 "forward" offsets
+// (dz = 0: right, and the three below; dz = +1: all nine).  Same 32 x 8 tile with a one-voxel halo as the gradient,
+// two z-planes; owners are the first S_own slices (slabs: the slice above the core is only a neighbour).
 __global__ void __launch_bounds__(256) k_prior_value(const float *__restrict__ zv, PriorK pk, double *partials, int S, int n, int S_own) {
-    const size_t total = (size_t)S_own * n * n;      // pairs are owned by their lower slice; owners: the first S_own slices
+    __shared__ float t[2][10][34];
+    __shared__ double red[8];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int ntx = (n + 31) / 32, nty = (n + 7) / 8;
+    const long long ntiles = (long long)ntx * nty * S_own;
     double sum = 0.0;
-    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
-        const int x = (int)(i % n), yy = (int)((i / n) % n), s = (int)(i / ((size_t)n * n));
-        const float c0 = zv[i];
-        float acc = 0.f;
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int s = (int)(tile / (ntx * nty)), r = (int)(tile % (ntx * nty));
+        const int x0 = (r % ntx) * 32, y0 = (r / ntx) * 8;
+        __syncthreads();
+        for (int e = threadIdx.x; e < 2 * 10 * 34; e += 256) {
+            const int dz = e / 340, q = e % 340, yy = q / 34, xx = q % 34;
+            const int gz = s + dz, gy = y0 + yy - 1, gx = x0 + xx - 1;
+            const bool in = gz < S && gy >= 0 && gy < n && gx >= 0 && gx < n;
+            t[dz][yy][xx] = in ? zv[((size_t)gz * n + gy) * n + gx] : __int_as_float(0x7fc00000);   // NaN marks "outside"
+        }
+        __syncthreads();
+        if (x0 + tx < n && y0 + ty < n) {
+            const float c0 = t[0][ty + 1][tx + 1];
+            float acc = 0.f;
 #pragma unroll
-        for (int dz = 0; dz <= 1; ++dz)
+            for (int dz = 0; dz <= 1; ++dz)
 #pragma unroll
-            for (int dy = -1; dy <= 1; ++dy)
+                for (int dy = -1; dy <= 1; ++dy)
 #pragma unroll
-                for (int dx = -1; dx <= 1; ++dx) {
-                    if (dz == 0 && (dy < 0 || (dy == 0 && dx <= 0))) continue;
-                    const int gz = s + dz, gy = yy + dy, gx = x + dx;
-                    if (gz < S && gy >= 0 && gy < n && gx >= 0 && gx < n)
-                        acc = fmaf(wgt(dz, dy, dx), hval(c0 - __ldg(&zv[((size_t)gz * n + gy) * n + gx]), pk), acc);
-                }
-        sum += (double)acc;
+                    for (int dx = -1; dx <= 1; ++dx) {
+                        if (dz == 0 && (dy < 0 || (dy == 0 && dx <= 0))) continue;
+                        const float v = t[dz][ty + 1 + dy][tx + 1 + dx];
+                        if (v == v) acc = fmaf(wgt(dz, dy, dx), hval(c0 - v, pk), acc);
+                    }
+            sum += (double)acc;
+        }
     }
-    block_reduce_to(sum, partials);
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
+    if (tx == 0) red[ty] = sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double v = 0.0;
+        for (int k = 0; k < 8; ++k) v += red[k];
+        partials[blockIdx.x] = v;
+    }
 }
 
 // ---- wrappers -------------------------------------------------------------------------------------
