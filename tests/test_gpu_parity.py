@@ -264,3 +264,25 @@ def test_mbir_out_of_core_streaming_matches_in_core_and_oracle(tc):
     assert rel_l2(x_st, xo) < TOL_MBIR
     F = [l["F"] for l in log_st]
     assert all(F[i + 1] <= F[i] for i in range(len(F) - 1))
+
+
+def test_full_size_config3_and_config5_geometry_sampled(tc):
+    # BASELINE configs 3 (1024^2, 128 angles, porous cylinder + Poisson noise) and 5 (2560^2 = 2^9 * 5, 1313 angles) in the launch
+    # configuration the library uses for them (compile-time pass lists, radix-5 last pass at 2560): 8 slices, one slice against the
+    # full oracle NUFFT, a few angles against the direct DFT, adjoint identity on all 8.
+    from paper_2304_12934_b200 import inputs
+    from oracle import nufft, direct
+    for cfg, sel in ((3, [5, 77]), (5, [611])):
+        c = inputs.CONFIGS[cfg]
+        ang = inputs.angles_uniform(c["Na"]); a64 = ang.astype(np.float64)
+        vol = inputs.volume_porous(8, c["N"], c["seed"]) if cfg == 3 else inputs.volume_fibres(8, c["N"], c["seed"], n_fibres=400)
+        plan = tc.Plan(c["N"], c["Nd"], ang, c["centre"])
+        s = _np(plan.radon(_cuda(vol)))
+        so = nufft.radon_nufft(vol[3], a64, c["Nd"], c["centre"])
+        assert rel_l2(s[3], so) < TOL_NUFFT
+        assert rel_l2(s[3][sel], direct.radon_direct(vol[3], a64[sel], c["Nd"], c["centre"])) < TOL_DIRECT
+        y = inputs.poisson_sinogram(s, seed=19) if cfg == 3 else np.random.default_rng(20).standard_normal(s.shape).astype(np.float32)
+        b = _np(plan.backproject(_cuda(y)))
+        plan.close()
+        assert rel_l2(b[3], nufft.backproject_nufft(y[3], a64, c["N"], c["centre"])) < TOL_NUFFT
+        assert _adj_mismatch(vol, y, s, b) < TOL_ADJ
