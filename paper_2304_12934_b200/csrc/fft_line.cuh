@@ -20,23 +20,25 @@
 
 namespace tc {
 
-constexpr int LINE_THREADS = 512;
-constexpr int LINE_SLOTS = LINE_THREADS / 4;
+constexpr int LINE_SLOTS = 128;               // task slots per CTA; a CTA has LINE_SLOTS * PL threads (PL = planes it carries: 4 or 2)
+constexpr int LINE_THREADS = LINE_SLOTS * 4;    // the 4-plane form (polar kernels)
 
 __device__ __forceinline__ int pcell(int c) { return c + (c >> 4); }
 
 // Pass configuration: compile-time (every index, stride and radix folds to an immediate) for the sizes of the
 // BASELINE configs, run-time (from the descriptor) for everything else.  TWS = stride of the twiddle table.
-template <int N_, int TWS_, int... Rs> struct SCfg {
+template <int PL_, int N_, int TWS_, int... Rs> struct SCfg {
     static constexpr bool is_static = true;
+    static constexpr int PL = PL_;
     static constexpr int NP = sizeof...(Rs);
     __device__ __forceinline__ static constexpr int n() { return N_; }
     __device__ __forceinline__ static constexpr int tws() { return TWS_; }
     __device__ __forceinline__ static constexpr int npass() { return NP; }
     __device__ __forceinline__ static constexpr int radix(int i) { constexpr int r[NP] = {Rs...}; return r[i]; }
 };
-struct RCfg {
+template <int PL_> struct RCfgT {
     static constexpr bool is_static = false;
+    static constexpr int PL = PL_;
     FftDesc d; int tws_;
     __device__ __forceinline__ int n() const { return d.n; }
     __device__ __forceinline__ int tws() const { return tws_; }
@@ -86,9 +88,9 @@ __device__ __forceinline__ void line_first(const LineCtx &c, const Cfg &cfg, LD 
         for (int j = 0; j < R; ++j) v[j] = ld(b + nb * j, R % 2 == 0 ? j < R / 2 : 2 * (b + nb * j) < cfg.n());
         Bfly<R, INV>::run(v);
         twiddle_mul<R, INV>(c.tw, b * cfg.tws(), v);
-        float2 *o = c.sm + pcell(R * b) * 4 + c.pl;   // R b is a multiple of R and R divides 16: k never crosses a padding cell
+        float2 *o = c.sm + pcell(R * b) * Cfg::PL + c.pl;   // R b is a multiple of R and R divides 16: k never crosses a padding cell
 #pragma unroll
-        for (int k = 0; k < R; ++k) o[k * 4] = v[k];
+        for (int k = 0; k < R; ++k) o[k * Cfg::PL] = v[k];
     }
     __syncthreads();
 }
@@ -103,13 +105,13 @@ __device__ __forceinline__ void line_first_smem(const LineCtx &c, const Cfg &cfg
 #pragma unroll 1
     for (int b = c.slot; b < nb; b += LINE_SLOTS) {
         float2 v[R];
-        float2 *o = c.sm + pcell(R * b) * 4 + c.pl;
+        float2 *o = c.sm + pcell(R * b) * Cfg::PL + c.pl;
 #pragma unroll
-        for (int j = 0; j < R; ++j) v[j] = o[j * 4];
+        for (int j = 0; j < R; ++j) v[j] = o[j * Cfg::PL];
         Bfly<R, INV>::run(v);
         twiddle_mul<R, INV>(c.tw, b * cfg.tws(), v);
 #pragma unroll
-        for (int k = 0; k < R; ++k) o[k * 4] = v[k];
+        for (int k = 0; k < R; ++k) o[k * Cfg::PL] = v[k];
     }
     __syncthreads();
 }
@@ -121,20 +123,20 @@ __device__ __forceinline__ void line_mid(const LineCtx &c, const Cfg &cfg, int s
     const int ni = n / s, sub = ni / R;                 // sub = n_i / R_i = range of b_i
     const int ntask = n / R;
     const bool fast = ((R1 * sub) & 15) == 0;
-    const int step = pcell(R1 * sub) * 4;
+    const int step = pcell(R1 * sub) * Cfg::PL;
 #pragma unroll 1
     for (int T = c.slot; T < ntask; T += LINE_SLOTS) {
         const int k1 = T % R1, rest = T / R1;
         const int outer = rest / sub, bi = rest - outer * sub;
         const int c0 = R1 * (outer * ni + bi) + k1;
         float2 v[R];
-        float2 *p0 = c.sm + pcell(c0) * 4 + c.pl;
+        float2 *p0 = c.sm + pcell(c0) * Cfg::PL + c.pl;
         if (fast) {
 #pragma unroll
             for (int j = 0; j < R; ++j) v[j] = p0[j * step];
         } else {
 #pragma unroll
-            for (int j = 0; j < R; ++j) v[j] = c.sm[pcell(c0 + j * R1 * sub) * 4 + c.pl];
+            for (int j = 0; j < R; ++j) v[j] = c.sm[pcell(c0 + j * R1 * sub) * Cfg::PL + c.pl];
         }
         Bfly<R, INV>::run(v);
         twiddle_mul<R, INV>(c.tw, bi * s * cfg.tws(), v);
@@ -143,7 +145,7 @@ __device__ __forceinline__ void line_mid(const LineCtx &c, const Cfg &cfg, int s
             for (int j = 0; j < R; ++j) p0[j * step] = v[j];
         } else {
 #pragma unroll
-            for (int j = 0; j < R; ++j) c.sm[pcell(c0 + j * R1 * sub) * 4 + c.pl] = v[j];
+            for (int j = 0; j < R; ++j) c.sm[pcell(c0 + j * R1 * sub) * Cfg::PL + c.pl] = v[j];
         }
     }
     __syncthreads();
@@ -160,7 +162,7 @@ template <int R, bool INV, class Cfg, class PRE, class ST>
 __device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, PRE pre, ST st) {
     const int n = cfg.n(), R1 = cfg.radix(0), ntask = n / R;
     const bool fast = (R1 & 15) == 0;
-    const int step = pcell(R1) * 4;
+    const int step = pcell(R1) * Cfg::PL;
 #pragma unroll 1
     for (int T = c.slot; T < ntask; T += LINE_SLOTS) {
         const int k1 = T % R1;
@@ -178,12 +180,12 @@ __device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, PRE 
 #pragma unroll
         for (int k = 0; k < R; ++k) old[k] = pre(T + ntask * k, R % 2 == 0 ? k < R / 2 : 2 * (T + ntask * k) < n);
         if (fast) {
-            const float2 *p0 = c.sm + pcell(c0) * 4 + c.pl;
+            const float2 *p0 = c.sm + pcell(c0) * Cfg::PL + c.pl;
 #pragma unroll
             for (int j = 0; j < R; ++j) v[j] = p0[j * step];
         } else {
 #pragma unroll
-            for (int j = 0; j < R; ++j) v[j] = c.sm[pcell(c0 + j * R1) * 4 + c.pl];
+            for (int j = 0; j < R; ++j) v[j] = c.sm[pcell(c0 + j * R1) * Cfg::PL + c.pl];
         }
         Bfly<R, INV>::run(v);
 #pragma unroll
@@ -191,9 +193,10 @@ __device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, PRE 
     }
 }
 
+template <class Cfg>
 __device__ __forceinline__ LineCtx line_ctx(float2 *sm, const float2 *tw) {
     LineCtx c;
-    c.sm = sm; c.tw = tw; c.pl = threadIdx.x & 3; c.slot = threadIdx.x >> 2;
+    c.sm = sm; c.tw = tw; c.pl = threadIdx.x % Cfg::PL; c.slot = threadIdx.x / Cfg::PL;
     return c;
 }
 
@@ -234,7 +237,7 @@ __device__ __forceinline__ void runtime_finish(const LineCtx &c, const Cfg &cfg,
 // A barrier must separate two transforms that use the same shared memory (the caller's job).
 template <bool INV, class Cfg, class LD, class PRE, class ST>
 __device__ __forceinline__ void fft_line(float2 *sm, const Cfg &cfg, const float2 *tw, LD ld, PRE pre, ST st) {
-    const LineCtx c = line_ctx(sm, tw);
+    const LineCtx c = line_ctx<Cfg>(sm, tw);
     if constexpr (Cfg::is_static) {
         line_first<Cfg::radix(0), INV>(c, cfg, ld);
         static_finish<INV, Cfg, 1, Cfg::radix(0)>(c, cfg, pre, st);
@@ -251,7 +254,7 @@ __device__ __forceinline__ void fft_line(float2 *sm, const Cfg &cfg, const float
 // shared (filled at line_input_cell positions and synchronised by the caller) -> FFT -> global.
 template <bool INV, class Cfg, class ST>
 __device__ __forceinline__ void fft_line_from_smem(float2 *sm, const Cfg &cfg, const float2 *tw, ST st) {
-    const LineCtx c = line_ctx(sm, tw);
+    const LineCtx c = line_ctx<Cfg>(sm, tw);
     if constexpr (Cfg::is_static) {
         line_first_smem<Cfg::radix(0), INV>(c, cfg);
         static_finish<INV, Cfg, 1, Cfg::radix(0)>(c, cfg, NoPre(), st);

@@ -38,7 +38,10 @@ __device__ __forceinline__ int wrap(int i, int G) { return i < 0 ? i + G : (i >=
 //   grid     grid[g][x][y & 1][y >> 1]        column-major: F2 writes and B3 reads whole columns contiguously; the
 //                                             polar kernels address single cells and do not care
 //   adjoint  rowbuf[g][x][i]                  columns written contiguously (B3), rows read with a column stride (B3 rows)
-#define TC_LB __launch_bounds__(LINE_THREADS, 2)
+#define TC_LB __launch_bounds__(LINE_THREADS, 2)           // 4-plane CTAs (polar kernels): 512 threads
+// row / column kernels: 4-plane CTAs (512 threads, two per SM) or 2-plane CTAs (256 threads, 35 KB of shared memory, four per SM;
+// each CTA then touches 16-byte halves of the cells and the two CTAs of a line are launched next to each other)
+#define TC_LB2 __launch_bounds__(LINE_SLOTS * Cfg::PL, 8 / Cfg::PL)
 
 template <class Cfg> __device__ __forceinline__ Cfg make_cfg(const FftDesc &f, int tws) {
     if constexpr (Cfg::is_static) return Cfg{};
@@ -50,10 +53,11 @@ __device__ __forceinline__ Wrapped wrapped(int t, int n, bool lo) { const int h 
 
 // F1 + row FFT.  eq. (8) read backwards: g = f d(y_i) d(x_j), zero-padded to G at periodic index.
 template <class Cfg>
-__global__ void TC_LB k_fwd_rows(DevPlan d, const float *__restrict__ vol, int S, float2 *__restrict__ rowbuf) {
+__global__ void TC_LB2 k_fwd_rows(DevPlan d, const float *__restrict__ vol, int S, float2 *__restrict__ rowbuf) {
     float2 *sm = reinterpret_cast<float2 *>(smem_f4);
     const Cfg cfg = make_cfg<Cfg>(d.fN, 2);
-    const int i = blockIdx.x, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = threadIdx.x & 3;
+    constexpr int NH = 4 / Cfg::PL;                          // CTAs per line
+    const int i = blockIdx.x / NH, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = Cfg::PL * (blockIdx.x % NH) + threadIdx.x % Cfg::PL;
     const float di = d.deapod[i];
     const int sre = 8 * g + 2 * pl;
     const bool hre = sre < S, him = sre + 1 < S;
@@ -76,10 +80,11 @@ __global__ void TC_LB k_fwd_rows(DevPlan d, const float *__restrict__ vol, int S
 
 // F2 column FFT; only the n non-zero rows exist in rowbuf.
 template <class Cfg>
-__global__ void TC_LB k_fwd_cols(DevPlan d, const float2 *__restrict__ rowbuf, float2 *__restrict__ grid) {
+__global__ void TC_LB2 k_fwd_cols(DevPlan d, const float2 *__restrict__ rowbuf, float2 *__restrict__ grid) {
     float2 *sm = reinterpret_cast<float2 *>(smem_f4);
     const Cfg cfg = make_cfg<Cfg>(d.fN, 2);
-    const int x = blockIdx.x, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = threadIdx.x & 3;
+    constexpr int NH = 4 / Cfg::PL;                          // CTAs per line
+    const int x = blockIdx.x / NH, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = Cfg::PL * (blockIdx.x % NH) + threadIdx.x % Cfg::PL;
     const float2 *in = rowbuf + ((size_t)g * n * G + (size_t)(x & 1) * n + (x >> 1)) * 4 + pl;
     float2 *out = grid + ((size_t)g * G + x) * G * 4 + pl;
 #pragma unroll 1
@@ -98,10 +103,11 @@ __global__ void TC_LB k_fwd_cols(DevPlan d, const float2 *__restrict__ rowbuf, f
 
 // B3 inverse column FFT (unnormalised, eq. (8)); only the n rows of the crop are produced.
 template <class Cfg>
-__global__ void TC_LB k_adj_cols(DevPlan d, const float2 *__restrict__ grid, float2 *rowbuf) {
+__global__ void TC_LB2 k_adj_cols(DevPlan d, const float2 *__restrict__ grid, float2 *rowbuf) {
     float2 *sm = reinterpret_cast<float2 *>(smem_f4);
     const Cfg cfg = make_cfg<Cfg>(d.fN, 2);
-    const int x = blockIdx.x, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = threadIdx.x & 3;
+    constexpr int NH = 4 / Cfg::PL;                          // CTAs per line
+    const int x = blockIdx.x / NH, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = Cfg::PL * (blockIdx.x % NH) + threadIdx.x % Cfg::PL;
     const float2 *in = grid + ((size_t)g * G + x) * G * 4 + pl;
     float2 *out = rowbuf + ((size_t)g * G + x) * n * 4 + pl;                 // adjoint half-plane, column-major: [g][x][i]
 #pragma unroll 1
@@ -120,10 +126,11 @@ __global__ void TC_LB k_adj_cols(DevPlan d, const float2 *__restrict__ grid, flo
 
 // B3 inverse row FFT + B4 crop and deapodise ("division by phihat"); re -> slice 2 pl, im -> 2 pl + 1.
 template <class Cfg>
-__global__ void TC_LB k_adj_rows(DevPlan d, const float2 *__restrict__ rowbuf, int S, float *vol) {
+__global__ void TC_LB2 k_adj_rows(DevPlan d, const float2 *__restrict__ rowbuf, int S, float *vol) {
     float2 *sm = reinterpret_cast<float2 *>(smem_f4);
     const Cfg cfg = make_cfg<Cfg>(d.fN, 2);
-    const int i = blockIdx.x, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = threadIdx.x & 3;
+    constexpr int NH = 4 / Cfg::PL;                          // CTAs per line
+    const int i = blockIdx.x / NH, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = Cfg::PL * (blockIdx.x % NH) + threadIdx.x % Cfg::PL;
     const float2 *in = rowbuf + ((size_t)g * G * n + i) * 4 + pl;
     const float di = d.deapod[i];
     const int sre = 8 * g + 2 * pl;
