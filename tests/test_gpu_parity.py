@@ -255,11 +255,12 @@ def test_mbir_out_of_core_streaming_matches_in_core_and_oracle(tc):
     x_st, log_st = plan.mbir(b, pr, 6)                                        # forced streaming
     st = plan.sched_stats()
     plan.close()
-    assert st["n_slabs"] == 3 and st["h2d_bytes"] > 0 and st["d2h_bytes"] == 6 * (x_st.nbytes + b.nbytes)
-    assert rel_l2(x_st, x_in) <= 1e-6
+    assert st["n_slabs"] == 3 and st["h2d_bytes"] > 0 and st["d2h_bytes"] == 6 * x_st.nbytes
+    # the streamed loop recomputes A y, the in-core loop carries it by linearity: equal up to float32 rounding
+    assert rel_l2(x_st, x_in) <= 1e-5
     assert [l["accepted"] for l in log_st] == [l["accepted"] for l in log_in]
     for ls, li in zip(log_st, log_in):
-        assert abs(ls["F"] - li["F"]) <= 1e-9 * abs(li["F"])
+        assert abs(ls["F"] - li["F"]) <= 1e-6 * abs(li["F"])
     xo, logo = mbir.mbir(b, a64, n, 32.0, P, SIG, C, 1.0, L, 6)
     assert rel_l2(x_st, xo) < TOL_MBIR
     F = [l["F"] for l in log_st]
