@@ -48,6 +48,12 @@ template <class Cfg> __device__ __forceinline__ Cfg make_cfg(const FftDesc &f, i
     else return Cfg{f, tws};
 }
 
+// Only the disc of fine-grid cells within W/2 of some polar sample carries data: |kappa| < G/2, so cells with
+// kx^2 + ky^2 > (G/2 + 5)^2 (21 % of the grid) are never read by the gather nor written by the spread; the column
+// kernels neither store nor load them.  lim = (G/2 + 5)^2 - kx^2 for the column at hand.
+__device__ __forceinline__ int disc_limit(int x, int G) { const int kx = x < G / 2 ? x : x - G, R = G / 2 + 5; return R * R - kx * kx; }
+__device__ __forceinline__ bool disc_live(int y, int G, int lim) { const int ky = y < G / 2 ? y : y - G; return ky * ky <= lim; }
+
 struct Wrapped { int img, X; };      // image index and periodic fine-grid index of wrapped sample t (lo = t < n / 2)
 __device__ __forceinline__ Wrapped wrapped(int t, int n, bool lo) { const int h = n >> 1; Wrapped w; w.img = lo ? t + h : t - h; w.X = lo ? t : t + n; return w; }
 
@@ -87,6 +93,7 @@ __global__ void TC_LB2 k_fwd_cols(DevPlan d, const float2 *__restrict__ rowbuf, 
     const int x = blockIdx.x / NH, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = Cfg::PL * (blockIdx.x % NH) + threadIdx.x % Cfg::PL;
     const float2 *in = rowbuf + ((size_t)g * n * G + (size_t)(x & 1) * n + (x >> 1)) * 4 + pl;
     float2 *out = grid + ((size_t)g * G + x) * G * 4 + pl;
+    const int lim = disc_limit(x, G);
 #pragma unroll 1
     for (int p = 0; p < 2; ++p) {
         fft_line<false>(sm, cfg, d.twG,
@@ -96,7 +103,7 @@ __global__ void TC_LB2 k_fwd_cols(DevPlan d, const float2 *__restrict__ rowbuf, 
                 if (p) v = cmul(v, __ldg(&d.twG[w.X]));
                 return v;
             },
-            NoPre(), [&](int r, bool, float2 v, float2) { out[(p * n + r) * 4] = v; });
+            NoPre(), [&](int r, bool, float2 v, float2) { if (disc_live(2 * r + p, G, lim)) out[(p * n + r) * 4] = v; });
         __syncthreads();
     }
 }
@@ -110,10 +117,11 @@ __global__ void TC_LB2 k_adj_cols(DevPlan d, const float2 *__restrict__ grid, fl
     const int x = blockIdx.x / NH, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = Cfg::PL * (blockIdx.x % NH) + threadIdx.x % Cfg::PL;
     const float2 *in = grid + ((size_t)g * G + x) * G * 4 + pl;
     float2 *out = rowbuf + ((size_t)g * G + x) * n * 4 + pl;                 // adjoint half-plane, column-major: [g][x][i]
+    const int lim = disc_limit(x, G);
 #pragma unroll 1
     for (int p = 0; p < 2; ++p) {
         fft_line<true>(sm, cfg, d.twG,
-            [&](int k, bool) { return __ldg(&in[(p * n + k) * 4]); },
+            [&](int k, bool) { return disc_live(2 * k + p, G, lim) ? __ldg(&in[(p * n + k) * 4]) : make_float2(0.f, 0.f); },
             [&](int t, bool lo) { return p ? out[wrapped(t, n, lo).img * 4] : make_float2(0.f, 0.f); },   // this thread wrote it in phase 0
             [&](int t, bool lo, float2 v, float2 old) {
                 const Wrapped w = wrapped(t, n, lo);
