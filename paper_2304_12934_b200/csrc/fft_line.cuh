@@ -29,6 +29,7 @@ __device__ __forceinline__ int pcell(int c) { return c + (c >> 4); }
 // BASELINE configs, run-time (from the descriptor) for everything else.  TWS = stride of the twiddle table.
 template <int PL_, int N_, int TWS_, int... Rs> struct SCfg {
     static constexpr bool is_static = true;
+    static constexpr bool PM_LAST = false;
     static constexpr int PL = PL_;
     static constexpr int NP = sizeof...(Rs);
     __device__ __forceinline__ static constexpr int n() { return N_; }
@@ -38,6 +39,7 @@ template <int PL_, int N_, int TWS_, int... Rs> struct SCfg {
 };
 template <int PL_> struct RCfgT {
     static constexpr bool is_static = false;
+    static constexpr bool PM_LAST = false;
     static constexpr int PL = PL_;
     FftDesc d; int tws_;
     __device__ __forceinline__ int n() const { return d.n; }
@@ -45,6 +47,11 @@ template <int PL_> struct RCfgT {
     __device__ __forceinline__ int npass() const { return d.npass; }
     __device__ __forceinline__ int radix(int i) const { return d.radix[i]; }
 };
+
+// Plane-major last pass: thread = (plane, slot) instead of (slot, plane), so a warp's stores are 32 consecutive outputs of ONE
+// plane (a full 128-byte line per float slice) -- for kernels whose output is the float volume, at the price of 4-way bank
+// conflicts on that pass's shared-memory reads.
+template <class Base> struct PlaneMajorLast : Base { static constexpr bool PM_LAST = true; };
 
 struct LineCtx {
     float2 *sm;               // [padded cell][4 planes]
@@ -163,8 +170,9 @@ __device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, PRE 
     const int n = cfg.n(), R1 = cfg.radix(0), ntask = n / R;
     const bool fast = (R1 & 15) == 0;
     const int step = pcell(R1) * Cfg::PL;
+    const int my_pl = Cfg::PM_LAST ? threadIdx.x / LINE_SLOTS : c.pl, my_slot = Cfg::PM_LAST ? threadIdx.x % LINE_SLOTS : c.slot;
 #pragma unroll 1
-    for (int T = c.slot; T < ntask; T += LINE_SLOTS) {
+    for (int T = my_slot; T < ntask; T += LINE_SLOTS) {
         const int k1 = T % R1;
         int rem = T / R1, mult = n / R1, B0 = 0;
 #pragma unroll
@@ -180,12 +188,12 @@ __device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, PRE 
 #pragma unroll
         for (int k = 0; k < R; ++k) old[k] = pre(T + ntask * k, R % 2 == 0 ? k < R / 2 : 2 * (T + ntask * k) < n);
         if (fast) {
-            const float2 *p0 = c.sm + pcell(c0) * Cfg::PL + c.pl;
+            const float2 *p0 = c.sm + pcell(c0) * Cfg::PL + my_pl;
 #pragma unroll
             for (int j = 0; j < R; ++j) v[j] = p0[j * step];
         } else {
 #pragma unroll
-            for (int j = 0; j < R; ++j) v[j] = c.sm[pcell(c0 + j * R1) * Cfg::PL + c.pl];
+            for (int j = 0; j < R; ++j) v[j] = c.sm[pcell(c0 + j * R1) * Cfg::PL + my_pl];
         }
         Bfly<R, INV>::run(v);
 #pragma unroll

@@ -45,7 +45,7 @@ __device__ __forceinline__ int wrap(int i, int G) { return i < 0 ? i + G : (i >=
 
 template <class Cfg> __device__ __forceinline__ Cfg make_cfg(const FftDesc &f, int tws) {
     if constexpr (Cfg::is_static) return Cfg{};
-    else return Cfg{f, tws};
+    else { Cfg c; c.d = f; c.tws_ = tws; return c; }
 }
 
 // Only the disc of fine-grid cells within W/2 of some polar sample carries data: |kappa| < G/2, so cells with
@@ -136,12 +136,13 @@ __global__ void TC_LB2 k_adj_cols(DevPlan d, const float2 *__restrict__ grid, fl
 template <class Cfg>
 __global__ void TC_LB2 k_adj_rows(DevPlan d, const float2 *__restrict__ rowbuf, int S, float *vol) {
     float2 *sm = reinterpret_cast<float2 *>(smem_f4);
-    const Cfg cfg = make_cfg<Cfg>(d.fN, 2);
+    const PlaneMajorLast<Cfg> cfg = make_cfg<PlaneMajorLast<Cfg>>(d.fN, 2);
     constexpr int NH = 4 / Cfg::PL;                          // CTAs per line
     const int i = blockIdx.x / NH, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = Cfg::PL * (blockIdx.x % NH) + threadIdx.x % Cfg::PL;
     const float2 *in = rowbuf + ((size_t)g * G * n + i) * 4 + pl;
     const float di = d.deapod[i];
-    const int sre = 8 * g + 2 * pl;
+    const int plo = Cfg::PL * (blockIdx.x % NH) + threadIdx.x / LINE_SLOTS;     // plane of this thread in the (plane-major) last pass
+    const int sre = 8 * g + 2 * plo;
     const bool hre = sre < S, him = sre + 1 < S;
     float *vre = vol + ((size_t)sre * n + i) * n, *vim = vre + (size_t)n * n;
 #pragma unroll 1
