@@ -109,84 +109,176 @@ __device__ __forceinline__ float wgt(int dz, int dy, int dx) {
     return k == 1 ? TC_W_FACE : (k == 2 ? TC_W_EDGE : TC_W_CORN);
 }
 
-// M2 + M3: g = atr + lambda grad H(y), z = y - g / L.  One thread per voxel, 32 x 8 tiles in-plane; the tile
-// and its one-voxel halo for the three z-planes are staged in shared memory.
-template <bool STEP>
-__global__ void __launch_bounds__(256) k_prior_grad(const float *__restrict__ y, const float *atr, PriorK pk, float lambda,
-                                                     float invL, float *g, float *__restrict__ z, int S, int n, int s_first) {
-    __shared__ float t[3][10][34];
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 8, s = blockIdx.z + s_first;
-    for (int e = threadIdx.x; e < 3 * 10 * 34; e += 256) {
-        const int dz = e / 340, r = e % 340, yy = r / 34, xx = r % 34;
-        const int gz = s + dz - 1, gy = y0 + yy - 1, gx = x0 + xx - 1;
-        const bool in = gz >= 0 && gz < S && gy >= 0 && gy < n && gx >= 0 && gx < n;
-        t[dz][yy][xx] = in ? y[((size_t)gz * n + gy) * n + gx] : __int_as_float(0x7fc00000);   // NaN marks "outside"
-    }
-    __syncthreads();
-    const int gx = x0 + tx, gy = y0 + ty;
-    if (gx >= n || gy >= n) return;
-    const float c0 = t[1][ty + 1][tx + 1];
-    float acc = 0.f;
-#pragma unroll
-    for (int dz = -1; dz <= 1; ++dz)
-#pragma unroll
-        for (int dy = -1; dy <= 1; ++dy)
-#pragma unroll
-            for (int dx = -1; dx <= 1; ++dx) {
-                if (dz == 0 && dy == 0 && dx == 0) continue;
-                const float v = t[dz + 1][ty + 1 + dy][tx + 1 + dx];
-                if (v == v) acc = fmaf(wgt(dz, dy, dx), dh(c0 - v, pk), acc);     // neighbours outside the volume skipped (G12)
-            }
-    const size_t o = ((size_t)s * n + gy) * n + gx;
-    const float gv = (atr ? atr[o] : 0.f) + lambda * acc;
-    g[o] = gv;
-    if (STEP) z[o] = fmaf(-invL, gv, c0);
-}
+// M2 + M3, pair-sharing form.  h' is odd, so the pair {m, n} gives +d to m and -d to n with d = w h'(y_m - y_n): every pair
+// is evaluated ONCE (13 "forward" pairs per voxel instead of 26; the evaluation costs three MUFU and bounds the kernel).
+// A CTA owns a 32 x 8 tile with a one-voxel halo ring (34 x 10 = 340 of its 352 threads, one thread per column) and marches
+// through a chunk of slices: at slice s a thread evaluates its 4 in-plane forward pairs and its 9 pairs with slice s + 1,
+// leaves d in shared memory for the partner (the in-plane ones are picked up in the same step, the 9 others in the next
+// step), and the interior threads write g and z.  One warm-up step below the chunk supplies the first slice's incoming pairs.
+constexpr int PM_ZC = 16;        // output slices per chunk
+constexpr int PM_THREADS = 352;
 
-// M4 prior term: H(z) = sum over unordered pairs, each counted once through its 13 "forward" offsets
-// (dz = 0: right, and the three below; dz = +1: all nine).  Same 32 x 8 tile with a one-voxel halo as the gradient,
-// two z-planes; owners are the first S_own slices (slabs: the slice above the core is only a neighbour).
-__global__ void __launch_bounds__(256) k_prior_value(const float *__restrict__ zv, PriorK pk, double *partials, int S, int n, int S_own) {
-    __shared__ float t[2][10][34];
-    __shared__ double red[8];
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    const int ntx = (n + 31) / 32, nty = (n + 7) / 8;
-    const long long ntiles = (long long)ntx * nty * S_own;
-    double sum = 0.0;
-    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int s = (int)(tile / (ntx * nty)), r = (int)(tile % (ntx * nty));
-        const int x0 = (r % ntx) * 32, y0 = (r / ntx) * 8;
-        __syncthreads();
-        for (int e = threadIdx.x; e < 2 * 10 * 34; e += 256) {
-            const int dz = e / 340, q = e % 340, yy = q / 34, xx = q % 34;
-            const int gz = s + dz, gy = y0 + yy - 1, gx = x0 + xx - 1;
-            const bool in = gz < S && gy >= 0 && gy < n && gx >= 0 && gx < n;
-            t[dz][yy][xx] = in ? zv[((size_t)gz * n + gy) * n + gx] : __int_as_float(0x7fc00000);   // NaN marks "outside"
+template <bool STEP>
+__global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__restrict__ y, const float *atr, PriorK pk, float lambda,
+                                                                 float invL, float *g, float *__restrict__ z, int S, int n, int s_first, int n_out) {
+    __shared__ float val[2][10][34];
+    __shared__ float din[4][10][34];
+    __shared__ float dup[2][9][10][34];
+    const int t = threadIdx.x, hx = t % 34, hy = t / 34;
+    const bool live = t < 340;
+    const int gx = blockIdx.x * 32 + hx - 1, gy = blockIdx.y * 8 + hy - 1;
+    const bool inplane = live && gx >= 0 && gx < n && gy >= 0 && gy < n;
+    const bool core = hx >= 1 && hx <= 32 && hy >= 1 && hy <= 8;
+    const bool interior = inplane && core;
+    const int zlo = s_first + blockIdx.z * PM_ZC, zhi = min(zlo + PM_ZC, s_first + n_out);
+    const int zstart = zlo > 0 ? zlo - 1 : 0;
+    const float NaN = __int_as_float(0x7fc00000);
+    const size_t plane = (size_t)n * n, pix = (size_t)gy * n + gx;
+    // which of this thread's 13 forward pairs exist: partner inside the tile array, inside the image, and not a pair of two
+    // halo voxels (those belong to other tiles).  Independent of z: computed once.
+    unsigned mask = 0;
+    {
+        int o = 0;
+        for (int dz = 0; dz <= 1; ++dz)
+            for (int dy = -1; dy <= 1; ++dy)
+                for (int dx = -1; dx <= 1; ++dx) {
+                    if (dz == 0 && (dy < 0 || (dy == 0 && dx <= 0))) continue;
+                    const int ny = hy + dy, nx = hx + dx, px = gx + dx, py = gy + dy;
+                    const bool pcore = nx >= 1 && nx <= 32 && ny >= 1 && ny <= 8;
+                    if (inplane && ny >= 0 && ny < 10 && nx >= 0 && nx < 34 && px >= 0 && px < n && py >= 0 && py < n && (core || pcore)) mask |= 1u << o;
+                    ++o;
+                }
+    }
+    // values are fetched two slices ahead, so a load has a whole step to arrive; two barriers per step
+    float c_cur = inplane ? y[(size_t)zstart * plane + pix] : NaN;
+    float c_nxt = (inplane && zstart + 1 < S) ? y[(size_t)(zstart + 1) * plane + pix] : NaN;
+    if (live) { val[zstart & 1][hy][hx] = c_cur; val[(zstart + 1) & 1][hy][hx] = c_nxt; }
+    for (int zz = zstart; zz < zhi; ++zz) {
+        const bool warm = zz < zlo;
+        const float c_nn = (inplane && zz + 2 < S && zz + 1 < zhi) ? y[(size_t)(zz + 2) * plane + pix] : NaN;
+        __syncthreads();                 // values of zz, zz + 1 visible; everybody is done with the previous step's din / dup
+        float acc = 0.f;
+        if (live) {
+            const unsigned mk = (warm ? mask & ~15u : mask) & (zz + 1 < S ? ~0u : 15u);     // no in-plane pairs in the warm-up step, no upward pairs at the top
+            const float *vc = &val[zz & 1][hy][hx], *vu = &val[(zz + 1) & 1][hy][hx];
+            int o = 0;
+#pragma unroll
+            for (int dy = 0; dy <= 1; ++dy)
+#pragma unroll
+                for (int dx = -1; dx <= 1; ++dx) {
+                    if (dy == 0 && dx <= 0) continue;
+                    float dv = 0.f;
+                    if (mk >> o & 1) dv = wgt(0, dy, dx) * dh(c_cur - vc[dy * 34 + dx], pk);
+                    din[o][hy][hx] = dv; acc += dv; ++o;
+                }
+#pragma unroll
+            for (int dy = -1; dy <= 1; ++dy)
+#pragma unroll
+                for (int dx = -1; dx <= 1; ++dx) {
+                    float dv = 0.f;
+                    if (mk >> o & 1) dv = wgt(1, dy, dx) * dh(c_cur - vu[dy * 34 + dx], pk);
+                    dup[zz & 1][o - 4][hy][hx] = dv; acc += dv; ++o;
+                }
         }
         __syncthreads();
-        if (x0 + tx < n && y0 + ty < n) {
-            const float c0 = t[0][ty + 1][tx + 1];
-            float acc = 0.f;
+        if (interior && !warm) {
+            int o = 0;
 #pragma unroll
+            for (int dy = 0; dy <= 1; ++dy)
+#pragma unroll
+                for (int dx = -1; dx <= 1; ++dx) {
+                    if (dy == 0 && dx <= 0) continue;
+                    acc -= din[o][hy - dy][hx - dx]; ++o;
+                }
+            if (zz > zstart) {                                    // the pairs with the slice below (none at the bottom of the volume)
+                o = 0;
+#pragma unroll
+                for (int dy = -1; dy <= 1; ++dy)
+#pragma unroll
+                    for (int dx = -1; dx <= 1; ++dx) { acc -= dup[(zz - 1) & 1][o][hy - dy][hx - dx]; ++o; }
+            }
+            const size_t oi = (size_t)zz * plane + pix;
+            const float gvv = (atr ? atr[oi] : 0.f) + lambda * acc;
+            g[oi] = gvv;
+            if (STEP) z[oi] = fmaf(-invL, gvv, c_cur);
+        }
+        c_cur = c_nxt; c_nxt = c_nn;
+        if (live) val[zz & 1][hy][hx] = c_nn;       // slice zz + 2 replaces slice zz (read before the barrier above)
+    }
+}
+
+// M4 prior term: H(z) = sum over unordered pairs, each counted once through its 13 "forward" offsets (dz = 0: right, and the
+// three below; dz = +1: all nine).  The same tiles and chunks as k_prior_grad_march, every plane is loaded once; a pair is owned
+// by its lower voxel, owners are the first S_own slices (slabs: the slice above the core is only a neighbour).  A fixed number of
+// CTAs walks the (tile, chunk) items, so the float64 partial sums and their final order are deterministic.
+__global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *__restrict__ zv, PriorK pk, double *partials, int S, int n, int S_own) {
+    __shared__ float val[2][10][34];
+    __shared__ double red[PM_THREADS / 32];
+    const int t = threadIdx.x, hx = t % 34, hy = t / 34;
+    const bool live = t < 340;
+    const bool core = hx >= 1 && hx <= 32 && hy >= 1 && hy <= 8;
+    const int ntx = (n + 31) / 32, nty = (n + 7) / 8, nch = (S_own + PM_ZC - 1) / PM_ZC;
+    const long long nitems = (long long)ntx * nty * nch;
+    const size_t plane = (size_t)n * n;
+    double sum = 0.0;
+    for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
+        const int ch = (int)(item / (ntx * nty)), r = (int)(item % (ntx * nty));
+        const int gx = (r % ntx) * 32 + hx - 1, gy = (r / ntx) * 8 + hy - 1;
+        const bool inplane = live && gx >= 0 && gx < n && gy >= 0 && gy < n;
+        unsigned mask = 0;
+        {
+            int o = 0;
             for (int dz = 0; dz <= 1; ++dz)
+                for (int dy = -1; dy <= 1; ++dy)
+                    for (int dx = -1; dx <= 1; ++dx) {
+                        if (dz == 0 && (dy < 0 || (dy == 0 && dx <= 0))) continue;
+                        const int px = gx + dx, py = gy + dy;
+                        if (inplane && core && px >= 0 && px < n && py >= 0 && py < n) mask |= 1u << o;
+                        ++o;
+                    }
+        }
+        const int zlo = ch * PM_ZC, zhi = min(zlo + PM_ZC, S_own);
+        const size_t pix = (size_t)gy * n + gx;
+        float c_cur = inplane ? zv[(size_t)zlo * plane + pix] : 0.f;
+        float c_nxt = (inplane && zlo + 1 < S) ? zv[(size_t)(zlo + 1) * plane + pix] : 0.f;
+        __syncthreads();                                    // the previous item's readers are done
+        if (live) { val[zlo & 1][hy][hx] = c_cur; val[(zlo + 1) & 1][hy][hx] = c_nxt; }
+        for (int zz = zlo; zz < zhi; ++zz) {
+            const float c_nn = (inplane && zz + 2 < S && zz + 1 < zhi) ? zv[(size_t)(zz + 2) * plane + pix] : 0.f;
+            __syncthreads();
+            const unsigned mk = mask & (zz + 1 < S ? ~0u : 15u);
+            if (mk) {
+                const float *vc = &val[zz & 1][hy][hx], *vu = &val[(zz + 1) & 1][hy][hx];
+                float acc = 0.f;
+                int o = 0;
+#pragma unroll
+                for (int dy = 0; dy <= 1; ++dy)
+#pragma unroll
+                    for (int dx = -1; dx <= 1; ++dx) {
+                        if (dy == 0 && dx <= 0) continue;
+                        if (mk >> o & 1) acc = fmaf(wgt(0, dy, dx), hval(c_cur - vc[dy * 34 + dx], pk), acc);
+                        ++o;
+                    }
 #pragma unroll
                 for (int dy = -1; dy <= 1; ++dy)
 #pragma unroll
                     for (int dx = -1; dx <= 1; ++dx) {
-                        if (dz == 0 && (dy < 0 || (dy == 0 && dx <= 0))) continue;
-                        const float v = t[dz][ty + 1 + dy][tx + 1 + dx];
-                        if (v == v) acc = fmaf(wgt(dz, dy, dx), hval(c0 - v, pk), acc);
+                        if (mk >> o & 1) acc = fmaf(wgt(1, dy, dx), hval(c_cur - vu[dy * 34 + dx], pk), acc);
+                        ++o;
                     }
-            sum += (double)acc;
+                sum += (double)acc;
+            }
+            __syncthreads();
+            c_cur = c_nxt; c_nxt = c_nn;
+            if (live) val[zz & 1][hy][hx] = c_nn;
         }
     }
     for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
-    if (tx == 0) red[ty] = sum;
+    if ((t & 31) == 0) red[t >> 5] = sum;
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (t == 0) {
         double v = 0.0;
-        for (int k = 0; k < 8; ++k) v += red[k];
+        for (int k = 0; k < PM_THREADS / 32; ++k) v += red[k];
         partials[blockIdx.x] = v;
     }
 }
@@ -204,9 +296,9 @@ void launch_residual(const float *Ax, const float *Axm, const float *b, float be
 void launch_update(const float *y, const float *atr, PriorDev pr, float invL, float *g, float *z, int S, int n, cudaStream_t st,
                    int s_first, int n_out) {
     if (n_out < 0) n_out = S - s_first;
-    dim3 gr((n + 31) / 32, (n + 7) / 8, n_out);
-    if (z) k_prior_grad<true><<<gr, 256, 0, st>>>(y, atr, mk(pr), pr.lambda, invL, g, z, S, n, s_first);
-    else   k_prior_grad<false><<<gr, 256, 0, st>>>(y, atr, mk(pr), pr.lambda, invL, g, nullptr, S, n, s_first);
+    dim3 gr((n + 31) / 32, (n + 7) / 8, (n_out + PM_ZC - 1) / PM_ZC);
+    if (z) k_prior_grad_march<true><<<gr, PM_THREADS, 0, st>>>(y, atr, mk(pr), pr.lambda, invL, g, z, S, n, s_first, n_out);
+    else   k_prior_grad_march<false><<<gr, PM_THREADS, 0, st>>>(y, atr, mk(pr), pr.lambda, invL, g, nullptr, S, n, s_first, n_out);
     TC_COUNT_LAUNCH();
 }
 void launch_candidate_sino(const float *Ay, const float *Ag, const float *b, float invL, float *Az, double *acc, size_t n, cudaStream_t st) {
@@ -217,7 +309,7 @@ void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, 
     if (S_own < 0) S_own = S;
     if (grad) { PriorDev p1 = pr; p1.lambda = 1.f; launch_update(z, nullptr, p1, 0.f, grad, nullptr, S, n, st); }
     if (acc) {
-        k_prior_value<<<RED_BLOCKS, RED_THREADS, 0, st>>>(z, mk(pr), acc + 16, S, n, S_own); TC_COUNT_LAUNCH();
+        k_prior_value_march<<<RED_BLOCKS, PM_THREADS, 0, st>>>(z, mk(pr), acc + 16, S, n, S_own); TC_COUNT_LAUNCH();
         final_reduce(acc, 1, 1.0, st);
     }
 }
