@@ -63,6 +63,14 @@ tc_status tc_radon(tc_plan *plan, const float *volume, int n_slices, float *sino
 /* volume[n_slices][n][n] = A^T sinogram[n_slices][n_angles][n_det]  (exact transpose of tc_radon). */
 tc_status tc_backproject(tc_plan *plan, const float *sinogram, int n_slices, float *volume, void *cuda_stream);
 
+/* Filtered back-projection, eq. (4) P:L64 (f = R* F^-1 |k| F p; filters P:L68): tc_backproject with every radial mode m weighted
+ * by (pi / n_angles) * r(m) * win(m), r = |m| / n_det (1 / (4 n_det) at m = 0, the mean of |k| over the DC bin), win = 1 for
+ * TC_FILTER_RAMP or 0.5 (1 + cos(2 pi m / n_det)) for TC_FILTER_HANN, so that tc_fbp(tc_radon(f)) ~ f for angles uniform in [0, pi).
+ * Same pointers, layouts, slab streaming and stream semantics as tc_backproject.  TC_EINVAL for an unknown filter. */
+#define TC_FILTER_RAMP 0
+#define TC_FILTER_HANN 1
+tc_status tc_fbp(tc_plan *plan, const float *sinogram, int n_slices, int filter, float *volume, void *cuda_stream);
+
 /* `iters` iterations of the monotone accelerated gradient method with restart on
  * F(f) = 1/2 ||A f - b||^2 + lambda H(f) from f = 0.  volume: out.  log: HOST pointer, nullable,
  * `iters` records.  Synchronous (returns when `volume` is complete). */

@@ -42,6 +42,7 @@ lib.tc_plan_create.argtypes = [ctypes.POINTER(tc_geom), _ci, ctypes.POINTER(_vp)
 lib.tc_plan_destroy.argtypes = [_vp]
 lib.tc_radon.argtypes = [_vp, _vp, _ci, _vp, _vp]
 lib.tc_backproject.argtypes = [_vp, _vp, _ci, _vp, _vp]
+lib.tc_fbp.argtypes = [_vp, _vp, _ci, _ci, _vp, _vp]
 lib.tc_mbir.argtypes = [_vp, _vp, _ci, ctypes.POINTER(tc_prior), _ci, _vp, ctypes.POINTER(tc_iter_log), _vp]
 lib.tc_power_iteration.argtypes = [_vp, _ci, ctypes.POINTER(ctypes.c_double)]
 lib.tc_prior_eval.argtypes = [_vp, _ci, _ci, ctypes.POINTER(tc_prior), _vp, ctypes.POINTER(ctypes.c_double)]
@@ -52,7 +53,7 @@ lib.tc_last_sched_stats.argtypes = [_vp, ctypes.POINTER(tc_sched_stats)]
 lib.tc_profile.argtypes = [_vp, _ci]
 lib.tc_profile_read.argtypes = [_vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_longlong)]
 lib.tc_last_error.restype = ctypes.c_char_p
-for _f in ("tc_plan_create", "tc_plan_destroy", "tc_radon", "tc_backproject", "tc_mbir", "tc_power_iteration",
+for _f in ("tc_plan_create", "tc_plan_destroy", "tc_radon", "tc_backproject", "tc_fbp", "tc_mbir", "tc_power_iteration",
            "tc_prior_eval", "tc_radon1", "tc_last_sched_stats", "tc_profile", "tc_profile_read"):
     getattr(lib, _f).restype = _ci
 
@@ -125,6 +126,13 @@ class Plan:
         assert tuple(sinogram.shape) == (S, self.n_angles, self.n_det)
         out = _like(sinogram, (S, self.n, self.n)) if out is None else out
         _check(lib.tc_backproject(self._h, _ptr(sinogram), S, _ptr(out), _stream(sinogram)))
+        return out
+
+    def fbp(self, sinogram, filter="ramp", out=None):
+        S = sinogram.shape[0]
+        assert tuple(sinogram.shape) == (S, self.n_angles, self.n_det)
+        out = _like(sinogram, (S, self.n, self.n)) if out is None else out
+        _check(lib.tc_fbp(self._h, _ptr(sinogram), S, {"ramp": 0, "hann": 1}[filter], _ptr(out), _stream(sinogram)))
         return out
 
     def mbir(self, sinogram, prior, iters, out=None):

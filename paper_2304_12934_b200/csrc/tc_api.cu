@@ -34,7 +34,8 @@ struct tc_plan {
     DevPlan d;
     int max_slab;                 // slices per slab (multiple of 8), 0 = not yet decided
     // device tables
-    float2 *twG = nullptr, *twD = nullptr, *ph_fwd = nullptr, *ph_adj = nullptr;
+    float2 *twG = nullptr, *twD = nullptr, *ph_fwd = nullptr, *ph_adj = nullptr, *ph_fbp[2] = {nullptr, nullptr};
+    int fbp_filter = 0;
     float *deapod = nullptr, *th_sorted = nullptr;
     double2 *cs = nullptr, *cs_sorted = nullptr;
     int *a_sorted = nullptr, *tile_nr = nullptr;
@@ -168,14 +169,20 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
         for (int i = 0; i < len; ++i) { const double a = 2.0 * M_PI * i / len; t[i] = make_float2((float)std::cos(a), (float)-std::sin(a)); }
         return t;
     };
-    std::vector<float2> phf(nd), pha(nd);
+    std::vector<float2> phf(nd), pha(nd), phr(nd), phh(nd);       // forward / adjoint phases; adjoint x FBP weights (ramp, Hann)
     const double centre = p->geom.center;
     for (int k = 0; k < nd; ++k) {
         const int m = k < nd / 2 ? k : k - nd;
-        if (k == nd / 2) { phf[k] = pha[k] = make_float2(0.f, 0.f); continue; }
+        if (k == nd / 2) { phf[k] = pha[k] = phr[k] = phh[k] = make_float2(0.f, 0.f); continue; }
         const double a = 2.0 * M_PI * std::fmod((double)m * centre, (double)nd) / nd;
         phf[k] = make_float2((float)(std::cos(a) / nd), (float)(-std::sin(a) / nd));
         pha[k] = make_float2((float)(std::cos(a) / nd), (float)(std::sin(a) / nd));
+        {   // eq. (4): |k| dk dtheta, the DC bin takes the mean of |k| over the bin
+            const double ramp = (M_PI / na) * (m == 0 ? 0.25 / nd : std::fabs((double)m) / nd);
+            const double hann = ramp * 0.5 * (1.0 + std::cos(2.0 * M_PI * m / nd));
+            phr[k] = make_float2((float)(ramp * std::cos(a) / nd), (float)(ramp * std::sin(a) / nd));
+            phh[k] = make_float2((float)(hann * std::cos(a) / nd), (float)(hann * std::sin(a) / nd));
+        }
     }
     std::vector<double2> cs(na), css(na);
     std::vector<float> ths(na);
@@ -196,6 +203,8 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
     if (e == cudaSuccess) e = upload(&p->twD, twd);
     if (e == cudaSuccess) e = upload(&p->ph_fwd, phf);
     if (e == cudaSuccess) e = upload(&p->ph_adj, pha);
+    if (e == cudaSuccess) e = upload(&p->ph_fbp[0], phr);
+    if (e == cudaSuccess) e = upload(&p->ph_fbp[1], phh);
     if (e == cudaSuccess) e = upload(&p->deapod, deapod);
     if (e == cudaSuccess) e = upload(&p->cs, cs);
     if (e == cudaSuccess) e = upload(&p->cs_sorted, css);
@@ -263,7 +272,7 @@ static void free_scratch(tc_plan *p) {
 extern "C" tc_status tc_plan_destroy(tc_plan *p) {
     if (!p) return TC_OK;
     free_scratch(p);
-    cudaFree(p->twG); cudaFree(p->twD); cudaFree(p->ph_fwd); cudaFree(p->ph_adj); cudaFree(p->deapod);
+    cudaFree(p->twG); cudaFree(p->twD); cudaFree(p->ph_fwd); cudaFree(p->ph_adj); cudaFree(p->ph_fbp[0]); cudaFree(p->ph_fbp[1]); cudaFree(p->deapod);
     cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc); cudaFree(p->tile_rng); cudaFree(p->tile_nr); cudaFree(p->tap_offs); cudaFree(p->taps); cudaFree(p->heavy);
     if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
     if (p->s_comp) cudaStreamDestroy(p->s_comp);
@@ -309,6 +318,16 @@ static void forward_slab(tc_plan *p, const float *vol, int S, float *sino, cudaS
     STAGE(0, launch_fwd_rows(p->d, vol, S, ng, p->rowbuf, st));
     STAGE(1, launch_fwd_cols(p->d, p->rowbuf, ng, p->grid, st));
     STAGE(2, launch_fwd_gather(p->d, p->grid, S, ng, sino, st));
+}
+// tc_fbp: the adjoint pipeline with the FBP-weighted phase table in place of ph_adj (one multiply in B1)
+static void fbp_slab(tc_plan *p, const float *sino, int S, float *vol, cudaStream_t st) {
+    const int ng = (S + 7) / 8;
+    DevPlan d2 = p->d;
+    d2.ph_adj = p->ph_fbp[p->fbp_filter];
+    STAGE(3, launch_adj_radial(d2, sino, S, ng, p->cpol, st));
+    STAGE(4, launch_adj_spread(p->d, p->cpol, ng, p->grid, st));
+    STAGE(5, launch_adj_cols(p->d, p->grid, ng, p->rowbuf, st));
+    STAGE(6, launch_adj_rows(p->d, p->rowbuf, S, ng, vol, st));
 }
 static void adjoint_slab(tc_plan *p, const float *sino, int S, float *vol, cudaStream_t st) {
     const int ng = (S + 7) / 8;

@@ -287,3 +287,30 @@ def test_full_size_config3_and_config5_geometry_sampled(tc):
         plan.close()
         assert rel_l2(b[3], nufft.backproject_nufft(y[3], a64, c["N"], c["centre"])) < TOL_NUFFT
         assert _adj_mismatch(vol, y, s, b) < TOL_ADJ
+
+
+def test_fbp_vs_oracle(tc):
+    # tc_fbp = the adjoint with ramp-weighted radial modes.  Against the oracle's NUFFT form and its definition,
+    # both filters, a ragged group and host pointers; and FBP(A f) ~ f on config 1's phantom.
+    from paper_2304_12934_b200 import inputs
+    from oracle import fbp
+    rng = np.random.default_rng(32)
+    S, n, nd, na, centre = 3, 64, 128, 40, 65.25
+    ang = inputs.angles_uniform(na); a64 = ang.astype(np.float64)
+    y = rng.standard_normal((S, na, nd)).astype(np.float32)
+    plan = tc.Plan(n, nd, ang, centre)
+    for w in ("ramp", "hann"):
+        f = _np(plan.fbp(_cuda(y), w))
+        assert rel_l2(f, fbp.fbp_nufft(y, a64, n, centre, w)) < TOL_NUFFT
+        assert rel_l2(f[1], fbp.fbp_direct(y[1], a64, n, centre, w)) < TOL_DIRECT
+    assert rel_l2(plan.fbp(y, "ramp"), _np(plan.fbp(_cuda(y), "ramp"))) <= 1e-6        # host pointers: slab scheduler
+    with pytest.raises(tc.TcError):
+        tc._check(tc.lib.tc_fbp(plan._h, tc._ptr(y), S, 7, tc._ptr(np.empty((S, n, n), np.float32)), None))
+    plan.close()
+    c = inputs.CONFIGS[1]
+    vol = inputs.volume_cfg1()
+    ang = inputs.angles_uniform(180)
+    plan = tc.Plan(c["N"], 256, ang, 128.0)
+    rec = _np(plan.fbp(plan.radon(_cuda(vol))))
+    plan.close()
+    assert rel_l2(rec, vol) < 0.15                                   # sharp-edged ellipses, band-limited reconstruction

@@ -213,3 +213,43 @@ def test_mbir_lambda0_meets_accelerated_rate_to_least_squares():
     g0 = np.linalg.norm(An.T @ b.ravel())
     assert np.linalg.norm(An.T @ (An @ x.ravel() - b.ravel())) < 0.02 * g0
     assert abs(log[-1]["F"] - 0.5 * np.sum((An @ x.ravel() - b.ravel()) ** 2)) < 1e-9 * log[-1]["F"]
+
+
+# ---- filtered back-projection (eq. (4)), oracle/fbp.py ------------------------------------------------------
+def test_fbp_reconstructs_gaussian_blob_closed_form():
+    # Continuous theory: FBP(R f) = f for band-limited f.  A Gaussian blob (s = 3 px) has the closed-form sinogram of
+    # oracle/analytic.py; with a detector 4x wider than the image the periodic wrap of the ramp is negligible, and what is left
+    # is a constant offset of order 1/Nd (the DC bin).  A wrong scale (pi/Na, 1/Nd), sign, axis or centre convention fails this.
+    from oracle import fbp, analytic
+    n, nd, na = 64, 256, 180
+    ang = np.arange(na) * np.pi / na
+    centre = nd / 2 + 0.25
+    x0, y0, s = 5.0, -7.0, 3.0
+    p = analytic.gaussian_projection(x0, y0, s, ang, nd, centre)
+    x = np.arange(n) - n // 2
+    truth = np.exp(-((x[None, :] - x0) ** 2 + (x[:, None] - y0) ** 2) / (2 * s * s))
+    f = fbp.fbp_direct(p, ang, n, centre, "ramp")
+    assert rel_l2(f, truth) < 5e-3
+    off = np.mean(f - truth)
+    assert rel_l2(f - off, truth) < 1e-4
+    fh = fbp.fbp_direct(p, ang, n, centre, "hann")              # Hann-apodised ramp: a slightly blurred blob, same place and mass
+    assert rel_l2(fh, truth) < 6e-2 and abs(fh.sum() / truth.sum() - 1.0) < 2e-2
+    iy, ix = np.unravel_index(np.argmax(fh), fh.shape)
+    assert (ix - n // 2, iy - n // 2) == (5, -7)
+
+
+def test_fbp_nufft_matches_definition_and_weights():
+    from oracle import fbp, direct
+    rng = np.random.default_rng(31)
+    n, nd, na = 32, 48, 21
+    ang = np.sort(rng.uniform(0, np.pi, na))
+    y = rng.standard_normal((2, na, nd))
+    for w in ("ramp", "hann"):
+        assert rel_l2(fbp.fbp_nufft(y, ang, n, 23.5, w), fbp.fbp_direct(y, ang, n, 23.5, w)) < 2e-5
+    rho = fbp.ramp_weights(nd, na)
+    m = np.arange(-(nd // 2) + 1, nd // 2)
+    assert np.allclose(rho[m != 0], np.pi / na * np.abs(m[m != 0]) / nd) and np.isclose(rho[m == 0][0], np.pi / na * 0.25 / nd)
+    # all weights equal to one turn FBP back into the plain adjoint (D2)
+    import unittest.mock as mock
+    with mock.patch.object(fbp, "ramp_weights", lambda nd_, na_, window="ramp": np.ones(nd_ - 1)):
+        assert rel_l2(fbp.fbp_direct(y, ang, n, 23.5), direct.backproject_direct(y, ang, n, 23.5)) < 1e-12
