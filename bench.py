@@ -233,7 +233,7 @@ def main():
         del hv, hs, hb
 
     if args.mbir:
-        Sm = min(S, 32)
+        Sm = S                                                     # the whole config: one MBIR iteration = 1 adjoint + 1 forward + update kernels
         b = sino[:Sm].contiguous()
         pr = tc.prior_params(L=float(1.05 * 1.02 * Na * N + 4.0 / (1e-4 * (1 / 0.7) ** 2)))
         plan.mbir(b, pr, 1); fence()
@@ -246,6 +246,8 @@ def main():
         t2, t8 = t_mbir(2), t_mbir(8)
         extra["mbir_iter_ms"] = 1e3 * (t8 - t2) / 6
         extra["mbir_pairs_per_s"] = Sm * Na / ((t8 - t2) / 6)
+        extra["mbir_model_bytes"] = (128 * N * N + 40 * Na * Nd) * Sm      # one MBIR iteration per slice
+        extra["mbir_frac_of_hbm_roofline"] = extra["mbir_model_bytes"] / ((t8 - t2) / 6) / 1e9 / peak
         extra["mbir_slices"] = Sm
 
     if args.ooc and rank == 0:
