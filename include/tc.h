@@ -42,8 +42,9 @@ typedef struct {
 /* qGGMRF prior h = (|D|/sigma)^2 / (c + (|D|/sigma)^(2-p)), eq. (13); paper's values
  * p = 1.2, sigma = 1/0.7, c = 1e-4.  lambda multiplies the prior (extension, default 1).
  * L is the step constant of the fixed 1/L step; 0 means: estimated by the library (power iteration
- * on A^T A plus the curvature bound of the prior, reading G15). */
-typedef struct { float p, sigma, c, lambda, L; } tc_prior;
+ * on A^T A plus the curvature bound of the prior, reading G15).  nonneg != 0 adds the constraint f >= 0 (P:L24:
+ * "the choice of the constraint is not limited by the algorithm design"): the candidate is projected, z = max(y - g/L, 0). */
+typedef struct { float p, sigma, c, lambda, L; int nonneg; } tc_prior;
 
 /* One record per MBIR iteration: F = objective of the kept iterate, data / prior = the two terms of
  * the CANDIDATE, margin = (F_prev - F_cand)/F_prev, beta = momentum used, accepted = 1/0. */

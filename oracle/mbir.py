@@ -23,8 +23,10 @@ def lipschitz(n, angles, nd, centre, p, sigma, c, lam, iters=10):
     return 1.05 * lam_hat + lam * 4.0 / (c * sigma * sigma), lam_hat
 
 
-def mbir(b, angles, n, centre, p, sigma, c, lam, L, iters, forced=None, keep_iterates=False):
-    """b: (S, Na, Nd).  Returns x (S, N, N), log (list of dicts), [iterates]."""
+def mbir(b, angles, n, centre, p, sigma, c, lam, L, iters, forced=None, keep_iterates=False, nonneg=False):
+    """b: (S, Na, Nd).  Returns x (S, N, N), log (list of dicts), [iterates].
+    nonneg: the candidate is projected on f >= 0 ("the choice of the constraint is not limited by the algorithm design",
+    P:L24): z = max(y - g/L, 0), the proximal-gradient step for the indicator of the positive orthant (G21)."""
     b = np.asarray(b, dtype=np.float64)
     S, na, nd = b.shape
     A = lambda f: nufft.radon_nufft(f, angles, nd, centre)
@@ -40,6 +42,8 @@ def mbir(b, angles, n, centre, p, sigma, c, lam, L, iters, forced=None, keep_ite
         Ay = A(y)
         g = At(Ay - b) + lam * prior.gradH(y, p, sigma, c)
         z = y - g / L
+        if nonneg:
+            z = np.maximum(z, 0.0)
         Az = A(z)
         data = 0.5 * np.sum((Az - b) ** 2)
         pri = prior.H(z, p, sigma, c)

@@ -23,7 +23,7 @@ class tc_geom(ctypes.Structure):
 
 class tc_prior(ctypes.Structure):
     _fields_ = [("p", ctypes.c_float), ("sigma", ctypes.c_float), ("c", ctypes.c_float),
-                ("lam", ctypes.c_float), ("L", ctypes.c_float)]
+                ("lam", ctypes.c_float), ("L", ctypes.c_float), ("nonneg", ctypes.c_int)]
 
 
 class tc_iter_log(ctypes.Structure):
@@ -92,8 +92,8 @@ def _like(a, shape):
     return torch.empty(shape, dtype=torch.float32, device=a.device, pin_memory=(not a.is_cuda and a.is_pinned()))
 
 
-def prior_params(p=1.2, sigma=1 / 0.7, c=1e-4, lam=1.0, L=0.0):
-    return tc_prior(p, sigma, c, lam, L)
+def prior_params(p=1.2, sigma=1 / 0.7, c=1e-4, lam=1.0, L=0.0, nonneg=False):
+    return tc_prior(p, sigma, c, lam, L, 1 if nonneg else 0)
 
 
 class Plan:

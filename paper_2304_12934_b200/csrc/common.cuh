@@ -58,7 +58,7 @@ void launch_adj_cols(const DevPlan &d, const float2 *grid, int ng, float2 *rowbu
 void launch_adj_rows(const DevPlan &d, const float2 *rowbuf, int S, int ng, float *vol, cudaStream_t st);
 
 // ---- kernels_mbir.cu -------------------------------------------------------------------------------
-struct PriorDev { float p, sigma, c, lambda; };
+struct PriorDev { float p, sigma, c, lambda; int nonneg = 0; };
 // y = x + beta (x - xm)                          (M1, volume part)
 void launch_extrapolate(const float *x, const float *xm, float beta, float *y, size_t n, cudaStream_t st);
 // r = Ax + beta (Ax - Axm) - b ; Ay kept          (M1, sinogram part)

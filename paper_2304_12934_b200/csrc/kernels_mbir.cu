@@ -80,7 +80,7 @@ __global__ void k_scale(float *v, float a, size_t n) {
 
 // ---- qGGMRF stencil -----------------------------------------------------------------------------
 // h(D) = u^2 / (c + u^(2-p)), h'(D) = sign(D)/sigma * u (2c + p u^(2-p)) / (c + u^(2-p))^2, u = |D|/sigma.
-struct PriorK { float inv_sigma, c, p, q; };     // q = 2 - p
+struct PriorK { float inv_sigma, c, p, q; int nonneg; };     // q = 2 - p; nonneg: project the candidate on z >= 0
 
 __device__ __forceinline__ float upow(float u, float q) {                                       // u >= 0; 0 -> 0 (lg2 -> -inf, ex2 -> 0)
     float r;
@@ -200,7 +200,7 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__
             const size_t oi = (size_t)zz * plane + pix;
             const float gvv = (atr ? atr[oi] : 0.f) + lambda * acc;
             g[oi] = gvv;
-            if (STEP) z[oi] = fmaf(-invL, gvv, c_cur);
+            if (STEP) { const float zc = fmaf(-invL, gvv, c_cur); z[oi] = pk.nonneg ? fmaxf(zc, 0.f) : zc; }
         }
         c_cur = c_nxt; c_nxt = c_nn;
         if (live) val[zz & 1][hy][hx] = c_nn;       // slice zz + 2 replaces slice zz (read before the barrier above)
@@ -285,7 +285,7 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *_
 
 // ---- wrappers -------------------------------------------------------------------------------------
 static int ew_blocks(size_t n) { size_t b = (n + 255) / 256; return (int)(b < 148 * 16 ? (b ? b : 1) : 148 * 16); }
-static PriorK mk(PriorDev pr) { PriorK k; k.inv_sigma = 1.f / pr.sigma; k.c = pr.c; k.p = pr.p; k.q = 2.f - pr.p; return k; }
+static PriorK mk(PriorDev pr) { PriorK k; k.inv_sigma = 1.f / pr.sigma; k.c = pr.c; k.p = pr.p; k.q = 2.f - pr.p; k.nonneg = pr.nonneg; return k; }
 
 void launch_extrapolate(const float *x, const float *xm, float beta, float *y, size_t n, cudaStream_t st) {
     k_extrapolate<<<ew_blocks(n), 256, 0, st>>>(x, xm, beta, y, n); TC_COUNT_LAUNCH();

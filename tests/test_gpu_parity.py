@@ -186,6 +186,31 @@ def test_mbir_config1_iterates(tc):
     assert all(F[i + 1] <= F[i] for i in range(len(F) - 1))
 
 
+def test_mbir_nonneg_constraint_vs_oracle(tc):
+    # the candidate projected on f >= 0 (A z recomputed, not carried by linearity); in core and streamed
+    from paper_2304_12934_b200 import inputs
+    from oracle import nufft, mbir
+    S, n, na = 10, 64, 24
+    ang = inputs.angles_uniform(na); a64 = ang.astype(np.float64)
+    vol = inputs.volume_cfg2(S=S, n=n)
+    # truth with a negative background, so that the unconstrained iterates go negative and the projection acts
+    b = (nufft.radon_nufft(vol - 0.25, a64, n, 32.0) + 0.05 * np.random.default_rng(34).standard_normal((S, na, n))).astype(np.float32)
+    L, _ = mbir.lipschitz(n, a64, n, 32.0, P, SIG, C, 1.0)
+    pr = tc.prior_params(P, SIG, C, 1.0, L, nonneg=True)
+    xo, logo = mbir.mbir(b, a64, n, 32.0, P, SIG, C, 1.0, L, 8, nonneg=True)
+    xu, _ = mbir.mbir(b, a64, n, 32.0, P, SIG, C, 1.0, L, 8)
+    assert xu.min() < -1e-3 and xo.min() >= 0.0                                # the constraint acts on this noisy data
+    for kw in ({}, {"max_slab_slices": 8}):
+        plan = tc.Plan(n, n, ang, 32.0, **kw)
+        x, log = plan.mbir(b if kw else _cuda(b), pr, 8)
+        x = x if kw else _np(x)
+        plan.close()
+        assert x.min() >= 0.0 and rel_l2(x, xo) < TOL_MBIR
+        assert [l["accepted"] for l in log] == [l["accepted"] for l in logo]
+        for lg, lo in zip(log, logo):
+            assert abs(lg["F"] - lo["F"]) < 1e-4 * abs(lo["F"])
+
+
 def test_mbir_multislice_with_noise(tc):
     # 11 slices (two groups, ragged) so the z-coupling of the 26-neighbour prior crosses a group boundary
     from paper_2304_12934_b200 import inputs

@@ -215,6 +215,32 @@ def test_mbir_lambda0_meets_accelerated_rate_to_least_squares():
     assert abs(log[-1]["F"] - 0.5 * np.sum((An @ x.ravel() - b.ravel()) ** 2)) < 1e-9 * log[-1]["F"]
 
 
+def test_mbir_nonneg_lambda0_converges_to_nnls():
+    # The constrained loop (G21) with lambda = 0 is accelerated projected gradient on 1/2||Ax-b||^2 over x >= 0,
+    # whose minimiser scipy's active-set NNLS computes from the brute-force dense matrix.  Data chosen so that the unconstrained
+    # least-squares solution has negative entries (otherwise the projection would never act).
+    from scipy.optimize import nnls
+    N, na = 8, 10
+    ang = np.arange(na) * math.pi / na
+    rng = np.random.default_rng(33)
+    b = rng.standard_normal((1, na, N))
+    An = np.stack([nufft.radon_nufft(e.reshape(N, N), ang, N, 4.0).ravel() for e in np.eye(N * N)], axis=1)
+    assert np.linalg.lstsq(An, b.ravel(), rcond=1e-10)[0].min() < -0.1
+    xs, rn = nnls(An, b.ravel())
+    Fstar = 0.5 * rn ** 2
+    Lc = 1.02 * np.linalg.norm(An, 2) ** 2
+    x, log, its = mbir.mbir(b, ang, N, 4.0, P, SIG, C, 0.0, Lc, 400, keep_iterates=True, nonneg=True)
+    assert all(it.min() >= 0.0 for it in its)
+    F = [l["F"] for l in log]
+    assert all(F[i + 1] <= F[i] for i in range(len(F) - 1))
+    assert Fstar - 1e-9 <= F[-1] <= Fstar * (1 + 1e-4) + 1e-9
+    assert (x > 0).sum() < N * N                                   # some constraints are active
+    # projected-gradient optimality (KKT): gradient >= 0 where x = 0, ~ 0 where x > 0
+    g = An.T @ (An @ x.ravel() - b.ravel())
+    g0 = np.linalg.norm(An.T @ b.ravel())
+    assert np.abs(g[x.ravel() > 1e-6]).max() < 0.02 * g0 and g[x.ravel() <= 1e-6].min() > -0.02 * g0
+
+
 # ---- filtered back-projection (eq. (4)), oracle/fbp.py ------------------------------------------------------
 def test_fbp_reconstructs_gaussian_blob_closed_form():
     # Continuous theory: FBP(R f) = f for band-limited f.  A Gaussian blob (s = 3 px) has the closed-form sinogram of
