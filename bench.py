@@ -243,11 +243,12 @@ def main():
             for _ in range(3):
                 t0 = time.perf_counter(); plan.mbir(b, pr, its); fence(); best = min(best, time.perf_counter() - t0)
             return best
-        t2, t8 = t_mbir(2), t_mbir(8)
-        extra["mbir_iter_ms"] = 1e3 * (t8 - t2) / 6
-        extra["mbir_pairs_per_s"] = Sm * Na / ((t8 - t2) / 6)
+        nit = int(min(300, max(6, 300.0 / (2.5 * ms_step))))       # enough iterations for ~0.3 s between the two timings
+        t2, t8 = t_mbir(2), t_mbir(2 + nit)
+        extra["mbir_iter_ms"] = 1e3 * (t8 - t2) / nit
+        extra["mbir_pairs_per_s"] = Sm * Na / ((t8 - t2) / nit)
         extra["mbir_model_bytes"] = (128 * N * N + 40 * Na * Nd) * Sm      # one MBIR iteration per slice
-        extra["mbir_frac_of_hbm_roofline"] = extra["mbir_model_bytes"] / ((t8 - t2) / 6) / 1e9 / peak
+        extra["mbir_frac_of_hbm_roofline"] = extra["mbir_model_bytes"] / ((t8 - t2) / nit) / 1e9 / peak
         extra["mbir_slices"] = Sm
 
     if args.ooc and rank == 0:
