@@ -20,7 +20,7 @@
 
 namespace tc {
 
-constexpr int LINE_SLOTS = 128;               // task slots per CTA; a CTA has LINE_SLOTS * PL threads (PL = planes it carries: 4 or 2)
+constexpr int LINE_SLOTS = 128;               // most task slots per CTA; a CTA has Cfg::SLOTS * PL threads (PL = planes it carries: 4 or 2)
 constexpr int LINE_THREADS = LINE_SLOTS * 4;    // the 4-plane form (polar kernels)
 
 __device__ __forceinline__ int pcell(int c) { return c + (c >> 4); }
@@ -31,6 +31,7 @@ template <int PL_, int N_, int TWS_, int... Rs> struct SCfg {
     static constexpr bool is_static = true;
     static constexpr bool PM_LAST = false;
     static constexpr int PL = PL_;
+    static constexpr int SLOTS = N_ / 16 < LINE_SLOTS ? (N_ / 16 < 32 ? 32 : N_ / 16) : LINE_SLOTS;   // one radix-16 task per thread when the line is short
     static constexpr int NP = sizeof...(Rs);
     __device__ __forceinline__ static constexpr int n() { return N_; }
     __device__ __forceinline__ static constexpr int tws() { return TWS_; }
@@ -41,6 +42,7 @@ template <int PL_> struct RCfgT {
     static constexpr bool is_static = false;
     static constexpr bool PM_LAST = false;
     static constexpr int PL = PL_;
+    static constexpr int SLOTS = LINE_SLOTS;
     FftDesc d; int tws_;
     __device__ __forceinline__ int n() const { return d.n; }
     __device__ __forceinline__ int tws() const { return tws_; }
@@ -89,7 +91,7 @@ template <int R, bool INV, class Cfg, class LD>
 __device__ __forceinline__ void line_first(const LineCtx &c, const Cfg &cfg, LD ld) {
     const int nb = cfg.n() / R;
 #pragma unroll 1
-    for (int b = c.slot; b < nb; b += LINE_SLOTS) {
+    for (int b = c.slot; b < nb; b += Cfg::SLOTS) {
         float2 v[R];
 #pragma unroll
         for (int j = 0; j < R; ++j) v[j] = ld(b + nb * j, R % 2 == 0 ? j < R / 2 : 2 * (b + nb * j) < cfg.n());
@@ -110,7 +112,7 @@ template <int R, bool INV, class Cfg>
 __device__ __forceinline__ void line_first_smem(const LineCtx &c, const Cfg &cfg) {
     const int nb = cfg.n() / R;
 #pragma unroll 1
-    for (int b = c.slot; b < nb; b += LINE_SLOTS) {
+    for (int b = c.slot; b < nb; b += Cfg::SLOTS) {
         float2 v[R];
         float2 *o = c.sm + pcell(R * b) * Cfg::PL + c.pl;
 #pragma unroll
@@ -132,7 +134,7 @@ __device__ __forceinline__ void line_mid(const LineCtx &c, const Cfg &cfg, int s
     const bool fast = ((R1 * sub) & 15) == 0;
     const int step = pcell(R1 * sub) * Cfg::PL;
 #pragma unroll 1
-    for (int T = c.slot; T < ntask; T += LINE_SLOTS) {
+    for (int T = c.slot; T < ntask; T += Cfg::SLOTS) {
         const int k1 = T % R1, rest = T / R1;
         const int outer = rest / sub, bi = rest - outer * sub;
         const int c0 = R1 * (outer * ni + bi) + k1;
@@ -170,9 +172,9 @@ __device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, PRE 
     const int n = cfg.n(), R1 = cfg.radix(0), ntask = n / R;
     const bool fast = (R1 & 15) == 0;
     const int step = pcell(R1) * Cfg::PL;
-    const int my_pl = Cfg::PM_LAST ? threadIdx.x / LINE_SLOTS : c.pl, my_slot = Cfg::PM_LAST ? threadIdx.x % LINE_SLOTS : c.slot;
+    const int my_pl = Cfg::PM_LAST ? threadIdx.x / Cfg::SLOTS : c.pl, my_slot = Cfg::PM_LAST ? threadIdx.x % Cfg::SLOTS : c.slot;
 #pragma unroll 1
-    for (int T = my_slot; T < ntask; T += LINE_SLOTS) {
+    for (int T = my_slot; T < ntask; T += Cfg::SLOTS) {
         const int k1 = T % R1;
         int rem = T / R1, mult = n / R1, B0 = 0;
 #pragma unroll

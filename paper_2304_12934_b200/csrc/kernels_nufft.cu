@@ -38,10 +38,10 @@ __device__ __forceinline__ int wrap(int i, int G) { return i < 0 ? i + G : (i >=
 //   grid     grid[g][x][y & 1][y >> 1]        column-major: F2 writes and B3 reads whole columns contiguously; the
 //                                             polar kernels address single cells and do not care
 //   adjoint  rowbuf[g][x][i]                  columns written contiguously (B3), rows read with a column stride (B3 rows)
-#define TC_LB __launch_bounds__(LINE_THREADS, 2)           // 4-plane CTAs (polar kernels): 512 threads
+#define TC_LB __launch_bounds__(Cfg::SLOTS * 4, 2)          // 4-plane CTAs (polar kernels): up to 512 threads
 // row / column kernels: 4-plane CTAs (512 threads, two per SM) or 2-plane CTAs (256 threads, 35 KB of shared memory, four per SM;
 // each CTA then touches 16-byte halves of the cells and the two CTAs of a line are launched next to each other)
-#define TC_LB2 __launch_bounds__(LINE_SLOTS * Cfg::PL, 8 / Cfg::PL)
+#define TC_LB2 __launch_bounds__(Cfg::SLOTS * Cfg::PL, 8 / Cfg::PL)
 
 template <class Cfg> __device__ __forceinline__ Cfg make_cfg(const FftDesc &f, int tws) {
     if constexpr (Cfg::is_static) return Cfg{};
@@ -141,7 +141,7 @@ __global__ void TC_LB2 k_adj_rows(DevPlan d, const float2 *__restrict__ rowbuf, 
     const int i = blockIdx.x / NH, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = Cfg::PL * (blockIdx.x % NH) + threadIdx.x % Cfg::PL;
     const float2 *in = rowbuf + ((size_t)g * G * n + i) * 4 + pl;
     const float di = d.deapod[i];
-    const int plo = Cfg::PL * (blockIdx.x % NH) + threadIdx.x / LINE_SLOTS;     // plane of this thread in the (plane-major) last pass
+    const int plo = Cfg::PL * (blockIdx.x % NH) + threadIdx.x / Cfg::SLOTS;     // plane of this thread in the (plane-major) last pass
     const int sre = 8 * g + 2 * plo;
     const bool hre = sre < S, him = sre + 1 < S;
     float *vre = vol + ((size_t)sre * n + i) * n, *vim = vre + (size_t)n * n;
