@@ -43,12 +43,14 @@ typedef struct {
  * p = 1.2, sigma = 1/0.7, c = 1e-4.  lambda multiplies the prior (extension, default 1).
  * L is the step constant of the fixed 1/L step; 0 means: estimated by the library (power iteration
  * on A^T A plus the curvature bound of the prior, reading G15).  nonneg != 0 adds the constraint f >= 0 (P:L24:
- * "the choice of the constraint is not limited by the algorithm design"): the candidate is projected, z = max(y - g/L, 0). */
-typedef struct { float p, sigma, c, lambda, L; int nonneg; } tc_prior;
+ * "the choice of the constraint is not limited by the algorithm design"): the candidate is projected, z = max(y - g/L, 0).
+ * grad_restart != 0 adds the gradient restart test: an accepted candidate with <g, z - x> > 0 resets the momentum. */
+typedef struct { float p, sigma, c, lambda, L; int nonneg, grad_restart; } tc_prior;
 
 /* One record per MBIR iteration: F = objective of the kept iterate, data / prior = the two terms of
- * the CANDIDATE, margin = (F_prev - F_cand)/F_prev, beta = momentum used, accepted = 1/0. */
-typedef struct { double F, data, prior, margin; float beta; int accepted; } tc_iter_log;
+ * the CANDIDATE, margin = (F_prev - F_cand)/F_prev, dot = <g, z - x> (0 unless grad_restart), beta = momentum used,
+ * accepted = 1/0, restarted = 1 if the gradient test reset the momentum. */
+typedef struct { double F, data, prior, margin, dot; float beta; int accepted, restarted; } tc_iter_log;
 
 typedef struct tc_plan tc_plan;
 

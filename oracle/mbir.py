@@ -23,10 +23,12 @@ def lipschitz(n, angles, nd, centre, p, sigma, c, lam, iters=10):
     return 1.05 * lam_hat + lam * 4.0 / (c * sigma * sigma), lam_hat
 
 
-def mbir(b, angles, n, centre, p, sigma, c, lam, L, iters, forced=None, keep_iterates=False, nonneg=False):
+def mbir(b, angles, n, centre, p, sigma, c, lam, L, iters, forced=None, keep_iterates=False, nonneg=False, grad_restart=False):
     """b: (S, Na, Nd).  Returns x (S, N, N), log (list of dicts), [iterates].
     nonneg: the candidate is projected on f >= 0 ("the choice of the constraint is not limited by the algorithm design",
-    P:L24): z = max(y - g/L, 0), the proximal-gradient step for the indicator of the positive orthant (G21)."""
+    P:L24): z = max(y - g/L, 0), the proximal-gradient step for the indicator of the positive orthant (G21).
+    grad_restart: the gradient restart test on top of the function-value test ("monotonic ... with restart"; DESIGN.md
+    G22): an accepted candidate with <g, z - x> > 0 (the step turned against the gradient at y) resets the momentum, t <- 1."""
     b = np.asarray(b, dtype=np.float64)
     S, na, nd = b.shape
     A = lambda f: nufft.radon_nufft(f, angles, nd, centre)
@@ -52,14 +54,16 @@ def mbir(b, angles, n, centre, p, sigma, c, lam, L, iters, forced=None, keep_ite
         accept = Fz <= Fx
         if forced is not None and it in forced:
             accept = bool(forced[it])
+        dot = float(np.sum(g * (z - x)))
+        restarted = bool(grad_restart and accept and dot > 0.0)
         if accept:
             xm, x = x, z
             Fx = Fz
-            t = tp
+            t = 1.0 if restarted else tp
         else:
             xm = x
             t = 1.0
-        log.append(dict(F=Fx, data=data, prior=pri, margin=margin, beta=beta, accepted=int(accept)))
+        log.append(dict(F=Fx, data=data, prior=pri, margin=margin, beta=beta, accepted=int(accept), restarted=int(restarted), dot=dot))
         if keep_iterates:
             its.append(x.copy())
     return (x, log, its) if keep_iterates else (x, log)

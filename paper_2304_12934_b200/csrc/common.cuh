@@ -74,6 +74,8 @@ void launch_candidate_sino(const float *Ay, const float *Ag, const float *b, flo
 void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, int n, cudaStream_t st, int S_own = -1);
 // acc[slot] += sum v^2
 void launch_sumsq(const float *v, size_t n, double *acc, int slot, cudaStream_t st);
+// acc[slot] += sum g (z - x)   (gradient restart test)
+void launch_dot_gzx(const float *g, const float *z, const float *x, size_t n, double *acc, int slot, cudaStream_t st);
 void launch_scale(float *v, float a, size_t n, cudaStream_t st);
 
 long long &launch_counter();

@@ -74,6 +74,12 @@ __global__ void k_sumsq(const float *__restrict__ v, size_t n, double *partials)
     }
     block_reduce_to(s, partials);
 }
+__global__ void k_dot_gzx(const float *__restrict__ g, const float *__restrict__ z, const float *__restrict__ x, size_t n, double *partials) {
+    double s = 0.0;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        s += (double)g[i] * ((double)z[i] - (double)x[i]);
+    block_reduce_to(s, partials);
+}
 __global__ void k_scale(float *v, float a, size_t n) {
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) v[i] *= a;
 }
@@ -82,9 +88,10 @@ __global__ void k_scale(float *v, float a, size_t n) {
 // h(D) = u^2 / (c + u^(2-p)), h'(D) = sign(D)/sigma * u (2c + p u^(2-p)) / (c + u^(2-p))^2, u = |D|/sigma.
 struct PriorK { float inv_sigma, c, p, q; int nonneg; };     // q = 2 - p; nonneg: project the candidate on z >= 0
 
-__device__ __forceinline__ float upow(float u, float q) {                                       // u >= 0; 0 -> 0 (lg2 -> -inf, ex2 -> 0)
+__device__ __forceinline__ float upow(float u, float q) {                                       // u^q, u >= 0: 0 -> 0 (lg2 -> -inf, ex2 -> 0)
     float r;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(q * __log2f(u)));
+    const float e = q == 0.f ? 0.f : q * __log2f(u);          // p = 2 (q = 0): u^0 = 1 also at u = 0 (0 * -inf would be NaN)
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(e));
     return r;
 }
 
@@ -315,6 +322,10 @@ void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, 
 }
 void launch_sumsq(const float *v, size_t n, double *acc, int slot, cudaStream_t st) {
     k_sumsq<<<RED_BLOCKS, RED_THREADS, 0, st>>>(v, n, acc + 16); TC_COUNT_LAUNCH();
+    final_reduce(acc, slot, 1.0, st);
+}
+void launch_dot_gzx(const float *g, const float *z, const float *x, size_t n, double *acc, int slot, cudaStream_t st) {
+    k_dot_gzx<<<RED_BLOCKS, RED_THREADS, 0, st>>>(g, z, x, n, acc + 16); TC_COUNT_LAUNCH();
     final_reduce(acc, slot, 1.0, st);
 }
 void launch_scale(float *v, float a, size_t n, cudaStream_t st) {

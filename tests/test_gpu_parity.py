@@ -145,9 +145,10 @@ def test_prior_kernels_vs_oracle(tc):
     for shape in ((1, 32, 32), (5, 64, 96)[:1] + (40, 40), (3, 33, 33)):
         v = (rng.standard_normal(shape) * rng.choice([0.01, 1.0, 30.0])).astype(np.float32)
         v[0, :4, :4] = 0.25                                                    # flat patch: h'(0) = 0 exactly
-        val, g = tc.prior_eval(_cuda(v), tc.prior_params(P, SIG, C))
-        assert abs(val - prior.H(v, P, SIG, C)) <= 2e-6 * prior.H(v, P, SIG, C)
-        assert rel_l2(_np(g), prior.gradH(v, P, SIG, C)) < 1e-5
+        for pp, ss, cc in ((P, SIG, C), (2.0, 1.0, 1.0)):                      # p = 2: the exponent 2 - p is 0 (u^0 at u = 0)
+            val, g = tc.prior_eval(_cuda(v), tc.prior_params(pp, ss, cc))
+            assert abs(val - prior.H(v, pp, ss, cc)) <= 2e-6 * prior.H(v, pp, ss, cc)
+            assert rel_l2(_np(g), prior.gradH(v, pp, ss, cc)) < 1e-5
     val, g = tc.prior_eval(_cuda(np.full((2, 32, 32), 0.7, np.float32)), tc.prior_params(P, SIG, C))
     assert val == 0.0 and np.all(_np(g) == 0.0)
 
@@ -207,6 +208,33 @@ def test_mbir_nonneg_constraint_vs_oracle(tc):
         plan.close()
         assert x.min() >= 0.0 and rel_l2(x, xo) < TOL_MBIR
         assert [l["accepted"] for l in log] == [l["accepted"] for l in logo]
+        for lg, lo in zip(log, logo):
+            assert abs(lg["F"] - lo["F"]) < 1e-4 * abs(lo["F"])
+
+
+def test_mbir_gradient_restart_vs_oracle(tc):
+    # gradient restart test.  Quadratic prior (p = 2) so that restarts occur within 30 iterations; the decision
+    # is the sign of <g, z - x>, compared where it is not a tie (|dot| above the float32 noise of the inner product)
+    from oracle import nufft, mbir
+    n, na = 32, 16
+    ang = (np.arange(na) * math.pi / na).astype(np.float32); a64 = ang.astype(np.float64)
+    rng = np.random.default_rng(35)
+    truth = np.zeros((2, n, n)); truth[:, 10:22, 8:20] = 1.0; truth[1, 14:18, 12:26] += 0.5
+    b = (nufft.radon_nufft(truth, a64, n, 16.0) + 0.01 * rng.standard_normal((2, na, n))).astype(np.float32)
+    p, sig, c, lam = 2.0, 1.0, 1.0, 200.0
+    L, _ = mbir.lipschitz(n, a64, n, 16.0, p, sig, c, lam)
+    xo, logo = mbir.mbir(b, a64, n, 16.0, p, sig, c, lam, L, 30, grad_restart=True)
+    assert sum(l["restarted"] for l in logo) >= 1
+    plan = tc.Plan(n, n, ang, 16.0)
+    x, log = plan.mbir(_cuda(b), tc.prior_params(p, sig, c, lam, L, grad_restart=True), 30)
+    x = _np(x); plan.close()
+    scale = max(abs(l["dot"]) for l in logo)
+    for lg, lo in zip(log, logo):
+        assert abs(lg["dot"] - lo["dot"]) <= 1e-3 * scale
+        if abs(lo["dot"]) > 2e-3 * scale:
+            assert lg["restarted"] == lo["restarted"] and lg["accepted"] == lo["accepted"]
+    if [l["restarted"] for l in log] == [l["restarted"] for l in logo]:
+        assert rel_l2(x, xo) < TOL_MBIR
         for lg, lo in zip(log, logo):
             assert abs(lg["F"] - lo["F"]) < 1e-4 * abs(lo["F"])
 

@@ -241,6 +241,30 @@ def test_mbir_nonneg_lambda0_converges_to_nnls():
     assert np.abs(g[x.ravel() > 1e-6]).max() < 0.02 * g0 and g[x.ravel() <= 1e-6].min() > -0.02 * g0
 
 
+def test_mbir_gradient_restart_variant():
+    # DESIGN.md G22 ("monotonic ... with restart"): on a strongly convex, well-conditioned objective (quadratic prior p = 2)
+    # plain accelerated gradient overshoots and the function-value test has to reject a candidate; the gradient test sees the
+    # overshoot first (<g, z - x> > 0), resets the momentum, and ends lower.  Checks the mechanics of the flag, not a number.
+    n, na = 32, 16
+    ang = np.arange(na) * math.pi / na
+    rng = np.random.default_rng(35)
+    truth = np.zeros((2, n, n)); truth[:, 10:22, 8:20] = 1.0; truth[1, 14:18, 12:26] += 0.5
+    b = nufft.radon_nufft(truth, ang, n, 16.0) + 0.01 * rng.standard_normal((2, na, n))
+    p, sig, c, lam = 2.0, 1.0, 1.0, 200.0
+    L, _ = mbir.lipschitz(n, ang, n, 16.0, p, sig, c, lam)
+    xr, lr = mbir.mbir(b, ang, n, 16.0, p, sig, c, lam, L, 60, grad_restart=True)
+    xp, lp = mbir.mbir(b, ang, n, 16.0, p, sig, c, lam, L, 60)
+    rs = [i for i, l in enumerate(lr) if l["restarted"]]
+    assert len(rs) >= 1 and all(lr[i]["accepted"] and lr[i]["dot"] > 0 for i in rs)
+    assert all(lr[i + 1]["beta"] == 0.0 for i in rs if i + 1 < len(lr))            # momentum reset: next step is a plain gradient step
+    assert all((l["dot"] > 0) == bool(l["restarted"]) for l in lr if l["accepted"])
+    F = [l["F"] for l in lr]
+    assert all(F[i + 1] <= F[i] for i in range(len(F) - 1))
+    assert any(not l["accepted"] for l in lp) and all(l["accepted"] for l in lr)     # the gradient test pre-empts the rejection
+    assert lr[-1]["F"] <= lp[-1]["F"]
+    assert all(l["restarted"] == 0 for l in lp) and lp[0]["dot"] == lr[0]["dot"]       # flag off: same loop as before
+
+
 # ---- filtered back-projection (eq. (4)), oracle/fbp.py ------------------------------------------------------
 def test_fbp_reconstructs_gaussian_blob_closed_form():
     # Continuous theory: FBP(R f) = f for band-limited f.  A Gaussian blob (s = 3 px) has the closed-form sinogram of
