@@ -1,8 +1,8 @@
-// Line FFT engine: one CTA transforms one line of P = 4 complex planes (a line of 32-byte cells), length
-// n = R1 R2 ... RL, with the first pass fused into the load and the last pass fused into the store.
+// Line FFT engine: one CTA transforms one line of PL complex planes (PL = 4: whole 32-byte cells; PL = 2: 16-byte halves of
+// them), length n = R1 R2 ... RL, with the first pass fused into the load and the last pass fused into the store.
 //
-// Thread t owns plane pl = t & 3 and task slot t >> 2: the four lanes of a quad touch the four 8-byte planes of
-// the same 32-byte cell in the same instruction, so every global access is a whole sector.  A task is one
+// Thread t owns plane pl = t % PL and task slot t / PL (SLOTS * PL threads): with PL = 4 the four lanes of a quad touch the four
+// 8-byte planes of the same 32-byte cell in the same instruction, so every global access is a whole sector.  A task is one
 // radix-R butterfly of one plane, held in registers; tasks of a pass are independent, a thread runs any number
 // of them one after the other, and there is one barrier per pass.
 //

@@ -21,7 +21,7 @@ extern __shared__ float4 smem_f4[];
 __device__ __forceinline__ int wrap(int i, int G) { return i < 0 ? i + G : (i >= G ? i - G : i); }
 
 // ------------------------------------------------------------------------------------------------
-// Line kernels: grid = (lines, groups); one CTA of LINE_THREADS = one line of the 4 planes of a group (fft_line.cuh).
+// Line kernels: grid = (lines x CTAs per line, groups); one CTA = one line of PL of the 4 planes of a group (fft_line.cuh).
 //
 // Pruned split.  The fine grid has G = 2 n points per axis but only n of them carry data on the image side
 // (zero padding, eq. (8)), so a length-G transform with n non-zero inputs is two length-n transforms:
@@ -29,8 +29,8 @@ __device__ __forceinline__ int wrap(int i, int G) { return i < 0 ? i + G : (i >=
 // where t < n runs over the image samples in wrapped order (t < n/2: image index t + n/2, periodic fine-grid
 // index X = t; t >= n/2: image index t - n/2, X = t + n).  The adjoint direction is the transpose: two length-n
 // inverse transforms of the even and odd inputs, the second multiplied by conj(mu_1) and added to the first.
-// A line therefore needs n (not G) cells of shared memory and two 512-thread CTAs fit on an SM, so one CTA's loads
-// overlap another's butterflies.
+// A line therefore needs n (not G) cells of shared memory (70 KB at n = 2048) and two 512-thread CTAs fit on an SM, so one
+// CTA's loads overlap another's butterflies.
 // Layouts (cells of P = 4 planes = 32 bytes): a sector-wide (32-byte) column access runs at 4.4 TB/s for loads but
 // 2.8 TB/s for stores on B200 (measured), so every store stream below is contiguous and only two load streams
 // are strided:
