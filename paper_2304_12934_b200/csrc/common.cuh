@@ -31,6 +31,8 @@ struct DevPlan {
     const int2 *taps;             // (a * nd + (m mod nd), float weight bits)
     const unsigned *heavy;        // [n_heavy] cells (cidx) whose list is longer than SPREAD_HEAVY
     unsigned n_heavy;
+    cudaStream_t side;            // the heavy-cell kernel runs beside the main spread kernel (disjoint cells): fork / join events
+    cudaEvent_t ev_fork, ev_join;
     int J;                        // radial modes to try on each side of the nearest one: floor(3 sqrt2 / sc + 1/2)
 };
 

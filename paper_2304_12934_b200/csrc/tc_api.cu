@@ -253,6 +253,12 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
             if (e == cudaSuccess) { launch_spread_heavy_list(d, (unsigned)nc, p->heavy, cnt, nullptr); e = cudaMemcpy(&d.n_heavy, cnt, sizeof(unsigned), cudaMemcpyDeviceToHost); }
             cudaFree(cnt);
             d.heavy = p->heavy;
+            d.side = nullptr; d.ev_fork = d.ev_join = nullptr;
+            if (e == cudaSuccess && d.n_heavy) {
+                e = cudaStreamCreateWithFlags(&d.side, cudaStreamNonBlocking);
+                if (e == cudaSuccess) e = cudaEventCreateWithFlags(&d.ev_fork, cudaEventDisableTiming);
+                if (e == cudaSuccess) e = cudaEventCreateWithFlags(&d.ev_join, cudaEventDisableTiming);
+            }
             if (e != cudaSuccess) { tc_plan_destroy(p); return fail(TC_ECUDA, std::string("spread heavy list: ") + cudaGetErrorString(e)); }
         }
         e = cudaDeviceSynchronize();
@@ -274,6 +280,9 @@ extern "C" tc_status tc_plan_destroy(tc_plan *p) {
     free_scratch(p);
     cudaFree(p->twG); cudaFree(p->twD); cudaFree(p->ph_fwd); cudaFree(p->ph_adj); cudaFree(p->ph_fbp[0]); cudaFree(p->ph_fbp[1]); cudaFree(p->deapod);
     cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc); cudaFree(p->tile_rng); cudaFree(p->tile_nr); cudaFree(p->tap_offs); cudaFree(p->taps); cudaFree(p->heavy);
+    if (p->d.side) cudaStreamDestroy(p->d.side);
+    if (p->d.ev_fork) cudaEventDestroy(p->d.ev_fork);
+    if (p->d.ev_join) cudaEventDestroy(p->d.ev_join);
     if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
     if (p->s_comp) cudaStreamDestroy(p->s_comp);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
