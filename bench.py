@@ -213,9 +213,17 @@ def main():
     # ---- e2e: host buffers through the C ABI (slab scheduler) ----
     e2e = None
     if not args.no_e2e:
-        hv = torch.from_numpy(vol_h).pin_memory()
-        hs = torch.empty((S, Na, Nd), dtype=torch.float32).pin_memory()
-        hb = torch.empty((S, N, N), dtype=torch.float32).pin_memory()
+        pinned = True
+        try:
+            hv = torch.from_numpy(vol_h).pin_memory()
+            hs = torch.empty((S, Na, Nd), dtype=torch.float32).pin_memory()
+            hb = torch.empty((S, N, N), dtype=torch.float32).pin_memory()
+        except Exception as exc:                                  # seen once right after an ncu run on the same box: fall back to pageable
+            sys.stderr.write("bench.py: pinning host buffers failed (%s); e2e uses pageable memory\n" % exc)
+            pinned = False
+            hv = torch.from_numpy(vol_h)
+            hs = torch.empty((S, Na, Nd), dtype=torch.float32)
+            hb = torch.empty((S, N, N), dtype=torch.float32)
         plan.radon(hv, out=hs); plan.backproject(hs, out=hb)      # warm-up (allocates staging)
         fence()
         t0 = time.perf_counter()
@@ -229,7 +237,7 @@ def main():
         bytes_out = hs.numel() * 4 + hb.numel() * 4
         e2e = {"value": world * S * Na / (t_e2e / args.steps), "unit": UNIT, "h2d_bytes_per_step": bytes_in, "d2h_bytes_per_step": bytes_out,
                "ms_per_step": 1e3 * t_e2e / args.steps, "pcie_GBps": (bytes_in + bytes_out) / (t_e2e / args.steps) / 1e9,
-               "overlap_mean": float(np.mean(ov))}
+               "overlap_mean": float(np.mean(ov)), "pinned_host_buffers": pinned}
         del hv, hs, hb
 
     if args.mbir:
