@@ -206,7 +206,8 @@ __device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, PRE 
 template <class Cfg>
 __device__ __forceinline__ LineCtx line_ctx(float2 *sm, const float2 *tw) {
     LineCtx c;
-    c.sm = sm; c.tw = tw; c.pl = threadIdx.x % Cfg::PL; c.slot = threadIdx.x / Cfg::PL;
+    c.sm = sm; c.tw = tw; c.pl = threadIdx.x % Cfg::PL;
+    c.slot = threadIdx.x < Cfg::SLOTS * Cfg::PL ? threadIdx.x / Cfg::PL : (1 << 30);      // a CTA may have more threads (the gather): they only meet the barriers
     return c;
 }
 
