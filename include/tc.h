@@ -11,9 +11,13 @@
  *   sinogram [slice][angle a][bin u]            (sinogram order), t_u = u - center
  * Pointers: every data pointer may be DEVICE memory or HOST memory (pinned or pageable); the
  *   library looks the pointer up (cudaPointerGetAttributes).  Host pointers take the slab-streaming
- *   path: slabs of slices go through pinned staging buffers on side streams, overlapped
- *   with compute, and the call returns when the output is complete.  Device-pointer calls are
- *   ordered on `cuda_stream` (a cudaStream_t, NULL = default stream) and return asynchronously.
+ *   path: slabs of slices go through device staging buffers on side streams, overlapped
+ *   with compute, and the call returns when the output is complete.  Pageable host arrays are page-locked
+ *   (cudaHostRegister) for the duration of the call so that their copies overlap; if that fails the call
+ *   still completes, without overlap.  Device-pointer calls are ordered on `cuda_stream` (a cudaStream_t,
+ *   NULL = default stream) and return asynchronously.
+ * Concurrency: a plan owns one set of scratch buffers, one side stream and its events: use it from one thread
+ *   and ONE stream at a time (two device-pointer calls on different streams would race on the scratch).
  * Ownership: the caller owns every data buffer; the plan owns all scratch; nothing allocated by the
  *   library is ever returned.  A plan is not thread-safe.
  * Errors: every call returns a tc_status; nothing throws or aborts across the ABI; outputs are
@@ -30,7 +34,8 @@ typedef enum { TC_OK = 0, TC_EINVAL = 1, TC_ENOMEM = 2, TC_ECUDA = 3, TC_EUNSUPP
 /* Acquisition geometry.  n: image side (even); n_det: detector bins (even); angles: HOST pointer to
  * n_angles float32 radians (copied at plan creation; any finite values); center: rotation-axis
  * position in bins (< 0 means n_det/2); oversamp must be 2.0 and kb_width 6 (Kaiser-Bessel
- * window; w ~ log10(1/eps)).  n must be a multiple of 32; 2n and n_det must be 2^a 5^b with b <= 1 (else TC_EUNSUPPORTED). */
+ * window; w ~ log10(1/eps)).  Sizes (else TC_EUNSUPPORTED): n and n_det must be multiples of 16 whose other prime factors
+ * are among 2, 3, 5, 7, 11, 13, 17 (e.g. 2048, 2560 = 2^9 5, 2448 = 2^4 3^2 17 of the paper's Table 1), at most 7000. */
 typedef struct {
     int n, n_det, n_angles;
     const float *angles;
@@ -44,13 +49,18 @@ typedef struct {
  * L is the step constant of the fixed 1/L step; 0 means: estimated by the library (power iteration
  * on A^T A plus the curvature bound of the prior, reading G15).  nonneg != 0 adds the constraint f >= 0 (P:L24:
  * "the choice of the constraint is not limited by the algorithm design"): the candidate is projected, z = max(y - g/L, 0).
- * grad_restart != 0 adds the gradient restart test: an accepted candidate with <g, z - x> > 0 resets the momentum. */
-typedef struct { float p, sigma, c, lambda, L; int nonneg, grad_restart; } tc_prior;
+ * grad_restart != 0 adds the gradient restart test: an accepted candidate with <g, z - x> > 0 resets the momentum.
+ * neighbours: the neighbour set of eq. (12): 26 (1-hop, the paper's; 0 means 26), 10 (the 8 in-plane neighbours and
+ * the 2 along z: the set P:L149 quotes for SVMBIR) or 6 (faces); weights 1/distance, normalised to sum 1 over the set.
+ * mm_step != 0 replaces the fixed step 1/L by the majorise-minimise step length along -g ("other optimizers"; G23):
+ * alpha = <g, g> / (||A g||^2 + lambda sum_pairs w h'(D)/D (g_m - g_n)^2), D = y_m - y_n; in-core problems only (TC_EUNSUPPORTED
+ * when the problem has to be streamed). */
+typedef struct { float p, sigma, c, lambda, L; int nonneg, grad_restart, neighbours, mm_step; } tc_prior;
 
 /* One record per MBIR iteration: F = objective of the kept iterate, data / prior = the two terms of
  * the CANDIDATE, margin = (F_prev - F_cand)/F_prev, dot = <g, z - x> (0 unless grad_restart), beta = momentum used,
- * accepted = 1/0, restarted = 1 if the gradient test reset the momentum. */
-typedef struct { double F, data, prior, margin, dot; float beta; int accepted, restarted; } tc_iter_log;
+ * accepted = 1/0, restarted = 1 if the gradient test reset the momentum, alpha = step length used (1/L unless mm_step). */
+typedef struct { double F, data, prior, margin, dot; float beta; int accepted, restarted; float alpha; } tc_iter_log;
 
 typedef struct tc_plan tc_plan;
 
@@ -76,7 +86,10 @@ tc_status tc_fbp(tc_plan *plan, const float *sinogram, int n_slices, int filter,
 
 /* `iters` iterations of the monotone accelerated gradient method with restart on
  * F(f) = 1/2 ||A f - b||^2 + lambda H(f) from f = 0.  volume: out.  log: HOST pointer, nullable,
- * `iters` records.  Synchronous (returns when `volume` is complete). */
+ * `iters` records.  Synchronous (returns when `volume` is complete).
+ * Device pointers: in core (4 volumes + 5 sinograms + FFT scratch of at most 128 slices in device memory; TC_ENOMEM if that
+ * does not fit).  Host pointers: in core if it fits, else streamed slab by slab (S1) with `volume` itself as one of
+ * the two host-resident volumes of the iteration and one more pinned by the library (n_slices n^2 floats). */
 tc_status tc_mbir(tc_plan *plan, const float *sinogram, int n_slices, const tc_prior *prior, int iters,
                   float *volume, tc_iter_log *log, void *cuda_stream);
 
@@ -94,9 +107,12 @@ tc_status tc_radon1(const float *volume, int n_slices, int n, const float *angle
 /* Kernel launches issued by this library on the calling thread since the last reset (for bench.py). */
 long long tc_launch_count(int reset);
 
-/* Scheduler statistics of the last host-pointer call: seconds of H2D, compute, D2H (summed CUDA-event
- * spans) and wall; overlap = (copy + compute - wall) / min(copy, compute). */
-typedef struct { double h2d_s, compute_s, d2h_s, wall_s, overlap; long long h2d_bytes, d2h_bytes; int n_slabs; } tc_sched_stats;
+/* Scheduler statistics of the last host-pointer call: seconds of H2D, compute, D2H (CUDA-event spans summed over the slabs; each
+ * stream is serial, so each is <= wall_s) and wall time of the streamed loop; overlap in [0, 1] =
+ * (h2d + compute + d2h - wall) / (h2d + compute + d2h - max(h2d, compute, d2h)): the fraction of the two shorter resources' work
+ * hidden behind the others (1: wall = the busiest resource alone; 0: no overlap).  setup_s: before the loop (page-locking,
+ * buffers, ||b||^2), handover_s: after it (copy into `volume` when x ended up in the library's buffer); both outside wall_s. */
+typedef struct { double h2d_s, compute_s, d2h_s, wall_s, overlap; long long h2d_bytes, d2h_bytes; int n_slabs; double setup_s, handover_s; } tc_sched_stats;
 tc_status tc_last_sched_stats(tc_plan *plan, tc_sched_stats *out);
 
 /* Per-kernel timing with CUDA events recorded on the launching stream around every NUFFT stage launch

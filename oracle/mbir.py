@@ -23,12 +23,18 @@ def lipschitz(n, angles, nd, centre, p, sigma, c, lam, iters=10):
     return 1.05 * lam_hat + lam * 4.0 / (c * sigma * sigma), lam_hat
 
 
-def mbir(b, angles, n, centre, p, sigma, c, lam, L, iters, forced=None, keep_iterates=False, nonneg=False, grad_restart=False):
+def mbir(b, angles, n, centre, p, sigma, c, lam, L, iters, forced=None, keep_iterates=False, nonneg=False, grad_restart=False,
+         neighbours=26, mm_step=False):
     """b: (S, Na, Nd).  Returns x (S, N, N), log (list of dicts), [iterates].
     nonneg: the candidate is projected on f >= 0 ("the choice of the constraint is not limited by the algorithm design",
     P:L24): z = max(y - g/L, 0), the proximal-gradient step for the indicator of the positive orthant (G21).
     grad_restart: the gradient restart test on top of the function-value test ("monotonic ... with restart"; DESIGN.md
-    G22): an accepted candidate with <g, z - x> > 0 (the step turned against the gradient at y) resets the momentum, t <- 1."""
+    G22): an accepted candidate with <g, z - x> > 0 (the step turned against the gradient at y) resets the momentum, t <- 1.
+    neighbours: neighbour set of the prior (oracle/prior.py).
+    mm_step: majorise-minimise step length along -g instead of the fixed 1/L ("other optimizers"; G23): the data
+    term is quadratic along the line, H is majorised by its symmetric-bound quadratic surrogate at y, and the step minimises the sum,
+        alpha = <g, g> / (||A g||^2 + lam curvH(y; g)),    z = y - alpha g.
+    (xm = x in the reject branch is implied by t = 1 -- the next step has beta = 0 -- and is kept for readability.)"""
     b = np.asarray(b, dtype=np.float64)
     S, na, nd = b.shape
     A = lambda f: nufft.radon_nufft(f, angles, nd, centre)
@@ -42,13 +48,17 @@ def mbir(b, angles, n, centre, p, sigma, c, lam, L, iters, forced=None, keep_ite
         beta = (t - 1.0) / tp
         y = x + beta * (x - xm)
         Ay = A(y)
-        g = At(Ay - b) + lam * prior.gradH(y, p, sigma, c)
-        z = y - g / L
+        g = At(Ay - b) + lam * prior.gradH(y, p, sigma, c, neighbours)
+        alpha = 1.0 / L
+        if mm_step:
+            den = np.sum(A(g) ** 2) + lam * prior.curvH(y, g, p, sigma, c, neighbours)
+            alpha = float(np.sum(g * g) / den) if den > 0.0 else 1.0 / L
+        z = y - alpha * g
         if nonneg:
             z = np.maximum(z, 0.0)
         Az = A(z)
         data = 0.5 * np.sum((Az - b) ** 2)
-        pri = prior.H(z, p, sigma, c)
+        pri = prior.H(z, p, sigma, c, neighbours)
         Fz = data + lam * pri
         margin = (Fx - Fz) / Fx
         accept = Fz <= Fx
@@ -63,7 +73,7 @@ def mbir(b, angles, n, centre, p, sigma, c, lam, L, iters, forced=None, keep_ite
         else:
             xm = x
             t = 1.0
-        log.append(dict(F=Fx, data=data, prior=pri, margin=margin, beta=beta, accepted=int(accept), restarted=int(restarted), dot=dot))
+        log.append(dict(F=Fx, data=data, prior=pri, margin=margin, beta=beta, accepted=int(accept), restarted=int(restarted), dot=dot, alpha=alpha))
         if keep_iterates:
             its.append(x.copy())
     return (x, log, its) if keep_iterates else (x, log)

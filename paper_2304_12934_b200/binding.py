@@ -23,19 +23,20 @@ class tc_geom(ctypes.Structure):
 
 class tc_prior(ctypes.Structure):
     _fields_ = [("p", ctypes.c_float), ("sigma", ctypes.c_float), ("c", ctypes.c_float),
-                ("lam", ctypes.c_float), ("L", ctypes.c_float), ("nonneg", ctypes.c_int), ("grad_restart", ctypes.c_int)]
+                ("lam", ctypes.c_float), ("L", ctypes.c_float), ("nonneg", ctypes.c_int), ("grad_restart", ctypes.c_int),
+                ("neighbours", ctypes.c_int), ("mm_step", ctypes.c_int)]
 
 
 class tc_iter_log(ctypes.Structure):
     _fields_ = [("F", ctypes.c_double), ("data", ctypes.c_double), ("prior", ctypes.c_double),
                 ("margin", ctypes.c_double), ("dot", ctypes.c_double), ("beta", ctypes.c_float), ("accepted", ctypes.c_int),
-                ("restarted", ctypes.c_int)]
+                ("restarted", ctypes.c_int), ("alpha", ctypes.c_float)]
 
 
 class tc_sched_stats(ctypes.Structure):
     _fields_ = [("h2d_s", ctypes.c_double), ("compute_s", ctypes.c_double), ("d2h_s", ctypes.c_double),
                 ("wall_s", ctypes.c_double), ("overlap", ctypes.c_double), ("h2d_bytes", ctypes.c_longlong),
-                ("d2h_bytes", ctypes.c_longlong), ("n_slabs", ctypes.c_int)]
+                ("d2h_bytes", ctypes.c_longlong), ("n_slabs", ctypes.c_int), ("setup_s", ctypes.c_double), ("handover_s", ctypes.c_double)]
 
 
 _vp, _ci = ctypes.c_void_p, ctypes.c_int
@@ -93,8 +94,8 @@ def _like(a, shape):
     return torch.empty(shape, dtype=torch.float32, device=a.device, pin_memory=(not a.is_cuda and a.is_pinned()))
 
 
-def prior_params(p=1.2, sigma=1 / 0.7, c=1e-4, lam=1.0, L=0.0, nonneg=False, grad_restart=False):
-    return tc_prior(p, sigma, c, lam, L, 1 if nonneg else 0, 1 if grad_restart else 0)
+def prior_params(p=1.2, sigma=1 / 0.7, c=1e-4, lam=1.0, L=0.0, nonneg=False, grad_restart=False, neighbours=26, mm_step=False):
+    return tc_prior(p, sigma, c, lam, L, 1 if nonneg else 0, 1 if grad_restart else 0, int(neighbours), 1 if mm_step else 0)
 
 
 class Plan:
@@ -142,7 +143,7 @@ class Plan:
         out = _like(sinogram, (S, self.n, self.n)) if out is None else out
         log = (tc_iter_log * max(iters, 1))()
         _check(lib.tc_mbir(self._h, _ptr(sinogram), S, ctypes.byref(prior), int(iters), _ptr(out), log, _stream(sinogram)))
-        recs = [dict(F=l.F, data=l.data, prior=l.prior, margin=l.margin, dot=l.dot, beta=l.beta, accepted=l.accepted, restarted=l.restarted)
+        recs = [dict(F=l.F, data=l.data, prior=l.prior, margin=l.margin, dot=l.dot, beta=l.beta, accepted=l.accepted, restarted=l.restarted, alpha=l.alpha)
                 for l in log[:iters]]
         return out, recs
 

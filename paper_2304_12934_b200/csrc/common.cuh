@@ -60,20 +60,26 @@ void launch_adj_cols(const DevPlan &d, const float2 *grid, int ng, float2 *rowbu
 void launch_adj_rows(const DevPlan &d, const float2 *rowbuf, int S, int ng, float *vol, cudaStream_t st);
 
 // ---- kernels_mbir.cu -------------------------------------------------------------------------------
-struct PriorDev { float p, sigma, c, lambda; int nonneg = 0; };
-// y = x + beta (x - xm)                          (M1, volume part)
+struct PriorDev { float p, sigma, c, lambda; int nonneg = 0; int nbr = 26; };   // nbr: neighbour set of eq. (12): 26 (paper), 10 or 6
+// y = x + beta (x - xm)                          (M1, volume part; only the streamed loop stores y)
 void launch_extrapolate(const float *x, const float *xm, float beta, float *y, size_t n, cudaStream_t st);
-// r = Ax + beta (Ax - Axm) - b ; Ay kept          (M1, sinogram part)
-void launch_residual(const float *Ax, const float *Axm, const float *b, float beta, float *Ay, float *r, size_t n, cudaStream_t st);
-// g = atr + lambda grad H(y);  z = y - g / L      (M2 + M3).  y has S slices of n x n; g may alias atr.
-// y has S slices; outputs are written for slices [s_first, s_first + n_out) only (n_out < 0: to the end) -- slabs with halos
-void launch_update(const float *y, const float *atr, PriorDev pr, float invL, float *g, float *z, int S, int n, cudaStream_t st,
-                   int s_first = 0, int n_out = -1);
-// Az = Ay - Ag / L;  acc[0] += 1/2 ||Az - b||^2   (M4 data term, fp64 accumulation)
-void launch_candidate_sino(const float *Ay, const float *Ag, const float *b, float invL, float *Az, double *acc, size_t n, cudaStream_t st);
-// acc[1] += H(z) over unordered 26-neighbour pairs (M4 prior term); grad (nullable) = grad H(z)
+// r = (Ax + beta (Ax - Axm)) - b                  (M1, sinogram part: A y is formed on the fly)
+void launch_residual(const float *Ax, const float *Axm, const float *b, float beta, float *r, size_t n, cudaStream_t st);
+// g = atr + lambda grad H(y);  z = y - g / L      (M2 + M3), y = x + beta (x - xm) formed on load (xm == nullptr: y = x).
+// g may alias atr; z == nullptr: gradient only.  y has S slices; outputs are written for slices [s_first, s_first + n_out) only
+// (n_out < 0: to the end) -- slabs with halos
+void launch_update(const float *x, const float *xm, float beta, const float *atr, PriorDev pr, float invL, float *g, float *z, int S, int n,
+                   cudaStream_t st, int s_first = 0, int n_out = -1);
+// z = y - alpha g (projected on z >= 0 if nonneg), y as above     (candidate of the majorise-minimise step)
+void launch_step(const float *x, const float *xm, float beta, const float *g, float alpha, int nonneg, float *z, size_t n, cudaStream_t st);
+// Az = Ay - alpha Ag, Ay = A0 + beta (A0 - A1) (A1 == nullptr: Ay = A0; Ag == nullptr: Az = Ay);  acc[0] += 1/2 ||Az - b||^2   (M4 data term)
+void launch_candidate_sino(const float *A0, const float *A1, const float *Ag, const float *b, float beta, float alpha, float *Az, double *acc,
+                           size_t n, cudaStream_t st);
+// acc[1] += H(z) over unordered neighbour pairs (M4 prior term); grad (nullable) = grad H(z)
 // pairs are owned by their lower slice; only owners among the first S_own slices are summed (S_own < 0: all)
 void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, int n, cudaStream_t st, int S_own = -1);
+// acc[slot] += sum over pairs of w h'(D)/D (g_m - g_n)^2, D = y_m - y_n, y = x + beta (x - xm)   (surrogate curvature along g)
+void launch_prior_curvature(const float *x, const float *xm, float beta, const float *g, PriorDev pr, double *acc, int slot, int S, int n, cudaStream_t st);
 // acc[slot] += sum v^2
 void launch_sumsq(const float *v, size_t n, double *acc, int slot, cudaStream_t st);
 // acc[slot] += sum g (z - x)   (gradient restart test)

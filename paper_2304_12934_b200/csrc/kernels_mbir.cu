@@ -2,6 +2,7 @@
 // (eqs. (12)-(13); 26 neighbours P:L149), gradient step and the objective's reductions.
 // Reductions accumulate in float64 and are deterministic: per-block partials, then one block adds them
 // to the accumulator slot.  Accumulator layout: acc[0..15] results, acc[16 .. 16+RED_BLOCKS) scratch.
+#include <cmath>
 #include "common.cuh"
 
 namespace tc {
@@ -46,25 +47,37 @@ __global__ void k_extrapolate(const float *__restrict__ x, const float *__restri
         y[i] = fmaf(beta, a - xm[i], a);
     }
 }
+// r = A y - b with A y = A x + beta (A x - A x-) formed on the fly (M1: the extrapolated sinogram is never stored)
 __global__ void k_residual(const float *__restrict__ Ax, const float *__restrict__ Axm, const float *__restrict__ b, float beta,
-                           float *__restrict__ Ay, float *__restrict__ r, size_t n) {
+                           float *__restrict__ r, size_t n) {
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         const float a = Ax[i];
-        const float ay = fmaf(beta, a - Axm[i], a);
-        Ay[i] = ay;
-        r[i] = ay - b[i];
+        r[i] = fmaf(beta, a - Axm[i], a) - b[i];
     }
 }
-__global__ void k_candidate_sino(const float *__restrict__ Ay, const float *__restrict__ Ag, const float *__restrict__ b, float invL,
-                                 float *__restrict__ Az, double *partials, size_t n) {
+// Az = A y - alpha A g (A y from A0, A1 as above; A1 == nullptr: A0 is A y itself; Ag == nullptr: Az = A y) and the data term.
+// No __restrict__: Az may alias any input (each thread reads its own elements before it writes them).
+__global__ void k_candidate_sino(const float *A0, const float *A1, const float *Ag, const float *b, float beta, float alpha,
+                                 float *Az, double *partials, size_t n) {
     double s = 0.0;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const float az = fmaf(-invL, Ag[i], Ay[i]);
+        const float a = A0[i];
+        const float ay = A1 ? fmaf(beta, a - A1[i], a) : a;
+        const float az = Ag ? fmaf(-alpha, Ag[i], ay) : ay;
         Az[i] = az;
         const double e = (double)az - (double)b[i];
         s += e * e;
     }
     block_reduce_to(s, partials);
+}
+// z = y - alpha g (projected on z >= 0 if nonneg), y = x + beta (x - x-): the candidate of the majorise-minimise step
+__global__ void k_step(const float *__restrict__ x, const float *__restrict__ xm, float beta, const float *__restrict__ g, float alpha,
+                       int nonneg, float *__restrict__ z, size_t n) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float a = x[i];
+        const float zc = fmaf(-alpha, g[i], fmaf(beta, a - xm[i], a));
+        z[i] = nonneg ? fmaxf(zc, 0.f) : zc;
+    }
 }
 __global__ void k_sumsq(const float *__restrict__ v, size_t n, double *partials) {
     double s = 0.0;
@@ -86,7 +99,9 @@ __global__ void k_scale(float *v, float a, size_t n) {
 
 // ---- qGGMRF stencil -----------------------------------------------------------------------------
 // h(D) = u^2 / (c + u^(2-p)), h'(D) = sign(D)/sigma * u (2c + p u^(2-p)) / (c + u^(2-p))^2, u = |D|/sigma.
-struct PriorK { float inv_sigma, c, p, q; int nonneg; };     // q = 2 - p; nonneg: project the candidate on z >= 0
+struct PriorK { float inv_sigma, c, p, q; int nonneg; unsigned allow; float wscale; };
+// q = 2 - p; nonneg: project the candidate on z >= 0; allow: which of the 13 forward offsets belong to the neighbour set (26: all;
+// 10: the 8 in-plane neighbours and the two along z; 6: faces), wscale: renormalises the 1/distance weights to sum 1 over the set
 
 __device__ __forceinline__ float upow(float u, float q) {                                       // u^q, u >= 0: 0 -> 0 (lg2 -> -inf, ex2 -> 0)
     float r;
@@ -105,6 +120,13 @@ __device__ __forceinline__ float dh(float D, const PriorK &k) {
 __device__ __forceinline__ float hval(float D, const PriorK &k) {
     const float u = fabsf(D) * k.inv_sigma;
     return __fdividef(u * u, k.c + upow(u, k.q));
+}
+// h'(D) / D = (2c + p u^q) / (sigma^2 (c + u^q)^2): the curvature of the quadratic surrogate of h at D (finite at D = 0: 2 / (c sigma^2))
+__device__ __forceinline__ float hcurv(float D, const PriorK &k) {
+    const float u = fabsf(D) * k.inv_sigma;
+    const float uq = upow(u, k.q);
+    const float den = k.c + uq;
+    return __fdividef(k.inv_sigma * k.inv_sigma * fmaf(k.p, uq, 2.f * k.c), den * den);
 }
 
 // w_mn = (1/dist) / (6 + 12/sqrt2 + 8/sqrt3)  (reading G10)
@@ -125,8 +147,10 @@ __device__ __forceinline__ float wgt(int dz, int dy, int dx) {
 constexpr int PM_ZC = 16;        // output slices per chunk
 constexpr int PM_THREADS = 352;
 
-template <bool STEP>
-__global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__restrict__ y, const float *atr, PriorK pk, float lambda,
+// The input is y = x + beta (x - x-), formed while loading when xm != nullptr (M1 fused: y never reaches HBM in the in-core loop).
+template <bool STEP, bool EXTRAP>
+__global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__restrict__ y, const float *__restrict__ xm, float beta,
+                                                                 const float *atr, PriorK pk, float lambda,
                                                                  float invL, float *g, float *__restrict__ z, int S, int n, int s_first, int n_out) {
     __shared__ float val[2][10][34];
     __shared__ float din[4][10][34];
@@ -155,14 +179,16 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__
                     if (inplane && ny >= 0 && ny < 10 && nx >= 0 && nx < 34 && px >= 0 && px < n && py >= 0 && py < n && (core || pcore)) mask |= 1u << o;
                     ++o;
                 }
+        mask &= pk.allow;
     }
+    auto ldy = [&](size_t i) { const float a = y[i]; return EXTRAP ? fmaf(beta, a - xm[i], a) : a; };
     // values are fetched two slices ahead, so a load has a whole step to arrive; two barriers per step
-    float c_cur = inplane ? y[(size_t)zstart * plane + pix] : NaN;
-    float c_nxt = (inplane && zstart + 1 < S) ? y[(size_t)(zstart + 1) * plane + pix] : NaN;
+    float c_cur = inplane ? ldy((size_t)zstart * plane + pix) : NaN;
+    float c_nxt = (inplane && zstart + 1 < S) ? ldy((size_t)(zstart + 1) * plane + pix) : NaN;
     if (live) { val[zstart & 1][hy][hx] = c_cur; val[(zstart + 1) & 1][hy][hx] = c_nxt; }
     for (int zz = zstart; zz < zhi; ++zz) {
         const bool warm = zz < zlo;
-        const float c_nn = (inplane && zz + 2 < S && zz + 1 < zhi) ? y[(size_t)(zz + 2) * plane + pix] : NaN;
+        const float c_nn = (inplane && zz + 2 < S && zz + 1 < zhi) ? ldy((size_t)(zz + 2) * plane + pix) : NaN;
         __syncthreads();                 // values of zz, zz + 1 visible; everybody is done with the previous step's din / dup
         float acc = 0.f;
         if (live) {
@@ -205,7 +231,7 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__
                     for (int dx = -1; dx <= 1; ++dx) { acc -= dup[(zz - 1) & 1][o][hy - dy][hx - dx]; ++o; }
             }
             const size_t oi = (size_t)zz * plane + pix;
-            const float gvv = (atr ? atr[oi] : 0.f) + lambda * acc;
+            const float gvv = (atr ? atr[oi] : 0.f) + lambda * pk.wscale * acc;
             g[oi] = gvv;
             if (STEP) { const float zc = fmaf(-invL, gvv, c_cur); z[oi] = pk.nonneg ? fmaxf(zc, 0.f) : zc; }
         }
@@ -218,8 +244,13 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__
 // three below; dz = +1: all nine).  The same tiles and chunks as k_prior_grad_march, every plane is loaded once; a pair is owned
 // by its lower voxel, owners are the first S_own slices (slabs: the slice above the core is only a neighbour).  A fixed number of
 // CTAs walks the (tile, chunk) items, so the float64 partial sums and their final order are deterministic.
-__global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *__restrict__ zv, PriorK pk, double *partials, int S, int n, int S_own) {
+// CURV = true: the curvature of the quadratic surrogate along a direction g instead (majorise-minimise step length):
+//   sum over pairs of w h'(D)/D (g_m - g_n)^2,  D = y_m - y_n,  y = x + beta (x - x-) formed on load.
+template <bool CURV>
+__global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *__restrict__ zv, const float *__restrict__ xm, float beta,
+                                                                  const float *__restrict__ gdir, PriorK pk, double *partials, int S, int n, int S_own) {
     __shared__ float val[2][10][34];
+    __shared__ float gval[CURV ? 2 : 1][CURV ? 10 : 1][CURV ? 34 : 1];
     __shared__ double red[PM_THREADS / 32];
     const int t = threadIdx.x, hx = t % 34, hy = t / 34;
     const bool live = t < 340;
@@ -227,6 +258,7 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *_
     const int ntx = (n + 31) / 32, nty = (n + 7) / 8, nch = (S_own + PM_ZC - 1) / PM_ZC;
     const long long nitems = (long long)ntx * nty * nch;
     const size_t plane = (size_t)n * n;
+    auto ldv = [&](size_t i) { const float a = zv[i]; return CURV ? fmaf(beta, a - xm[i], a) : a; };
     double sum = 0.0;
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int ch = (int)(item / (ntx * nty)), r = (int)(item % (ntx * nty));
@@ -243,19 +275,31 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *_
                         if (inplane && core && px >= 0 && px < n && py >= 0 && py < n) mask |= 1u << o;
                         ++o;
                     }
+            mask &= pk.allow;
         }
         const int zlo = ch * PM_ZC, zhi = min(zlo + PM_ZC, S_own);
         const size_t pix = (size_t)gy * n + gx;
-        float c_cur = inplane ? zv[(size_t)zlo * plane + pix] : 0.f;
-        float c_nxt = (inplane && zlo + 1 < S) ? zv[(size_t)(zlo + 1) * plane + pix] : 0.f;
+        float c_cur = inplane ? ldv((size_t)zlo * plane + pix) : 0.f;
+        float c_nxt = (inplane && zlo + 1 < S) ? ldv((size_t)(zlo + 1) * plane + pix) : 0.f;
+        float g_cur = 0.f, g_nxt = 0.f;
+        if (CURV) {
+            g_cur = inplane ? gdir[(size_t)zlo * plane + pix] : 0.f;
+            g_nxt = (inplane && zlo + 1 < S) ? gdir[(size_t)(zlo + 1) * plane + pix] : 0.f;
+        }
         __syncthreads();                                    // the previous item's readers are done
-        if (live) { val[zlo & 1][hy][hx] = c_cur; val[(zlo + 1) & 1][hy][hx] = c_nxt; }
+        if (live) {
+            val[zlo & 1][hy][hx] = c_cur; val[(zlo + 1) & 1][hy][hx] = c_nxt;
+            if (CURV) { gval[zlo & 1][hy][hx] = g_cur; gval[(zlo + 1) & 1][hy][hx] = g_nxt; }
+        }
         for (int zz = zlo; zz < zhi; ++zz) {
-            const float c_nn = (inplane && zz + 2 < S && zz + 1 < zhi) ? zv[(size_t)(zz + 2) * plane + pix] : 0.f;
+            const bool more = inplane && zz + 2 < S && zz + 1 < zhi;
+            const float c_nn = more ? ldv((size_t)(zz + 2) * plane + pix) : 0.f;
+            const float g_nn = (CURV && more) ? gdir[(size_t)(zz + 2) * plane + pix] : 0.f;
             __syncthreads();
             const unsigned mk = mask & (zz + 1 < S ? ~0u : 15u);
             if (mk) {
                 const float *vc = &val[zz & 1][hy][hx], *vu = &val[(zz + 1) & 1][hy][hx];
+                const float *gc = CURV ? &gval[zz & 1][hy][hx] : nullptr, *gu = CURV ? &gval[(zz + 1) & 1][hy][hx] : nullptr;
                 float acc = 0.f;
                 int o = 0;
 #pragma unroll
@@ -263,14 +307,20 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *_
 #pragma unroll
                     for (int dx = -1; dx <= 1; ++dx) {
                         if (dy == 0 && dx <= 0) continue;
-                        if (mk >> o & 1) acc = fmaf(wgt(0, dy, dx), hval(c_cur - vc[dy * 34 + dx], pk), acc);
+                        if (mk >> o & 1) {
+                            if (CURV) { const float dg = g_cur - gc[dy * 34 + dx]; acc = fmaf(wgt(0, dy, dx) * hcurv(c_cur - vc[dy * 34 + dx], pk), dg * dg, acc); }
+                            else acc = fmaf(wgt(0, dy, dx), hval(c_cur - vc[dy * 34 + dx], pk), acc);
+                        }
                         ++o;
                     }
 #pragma unroll
                 for (int dy = -1; dy <= 1; ++dy)
 #pragma unroll
                     for (int dx = -1; dx <= 1; ++dx) {
-                        if (mk >> o & 1) acc = fmaf(wgt(1, dy, dx), hval(c_cur - vu[dy * 34 + dx], pk), acc);
+                        if (mk >> o & 1) {
+                            if (CURV) { const float dg = g_cur - gu[dy * 34 + dx]; acc = fmaf(wgt(1, dy, dx) * hcurv(c_cur - vu[dy * 34 + dx], pk), dg * dg, acc); }
+                            else acc = fmaf(wgt(1, dy, dx), hval(c_cur - vu[dy * 34 + dx], pk), acc);
+                        }
                         ++o;
                     }
                 sum += (double)acc;
@@ -278,6 +328,7 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *_
             __syncthreads();
             c_cur = c_nxt; c_nxt = c_nn;
             if (live) val[zz & 1][hy][hx] = c_nn;
+            if (CURV) { g_cur = g_nxt; g_nxt = g_nn; if (live) gval[zz & 1][hy][hx] = g_nn; }
         }
     }
     for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
@@ -286,39 +337,61 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *_
     if (t == 0) {
         double v = 0.0;
         for (int k = 0; k < PM_THREADS / 32; ++k) v += red[k];
-        partials[blockIdx.x] = v;
+        partials[blockIdx.x] = v * (double)pk.wscale;
     }
 }
 
 // ---- wrappers -------------------------------------------------------------------------------------
 static int ew_blocks(size_t n) { size_t b = (n + 255) / 256; return (int)(b < 148 * 16 ? (b ? b : 1) : 148 * 16); }
-static PriorK mk(PriorDev pr) { PriorK k; k.inv_sigma = 1.f / pr.sigma; k.c = pr.c; k.p = pr.p; k.q = 2.f - pr.p; k.nonneg = pr.nonneg; return k; }
+// forward-offset order of the march kernels: o = 0..3 in plane (dy, dx) = (0, 1), (1, -1), (1, 0), (1, 1); o = 4..12: dz = 1, (dy, dx) row-major
+static PriorK mk(PriorDev pr) {
+    PriorK k; k.inv_sigma = 1.f / pr.sigma; k.c = pr.c; k.p = pr.p; k.q = 2.f - pr.p; k.nonneg = pr.nonneg;
+    const double s26 = 6.0 + 12.0 / std::sqrt(2.0) + 8.0 / std::sqrt(3.0);
+    if (pr.nbr == 10) { k.allow = 0xFu | (1u << 8); k.wscale = (float)(s26 / (6.0 + 4.0 / std::sqrt(2.0))); }       // 8 in plane + 2 along z
+    else if (pr.nbr == 6) { k.allow = (1u << 0) | (1u << 2) | (1u << 8); k.wscale = (float)(s26 / 6.0); }              // faces
+    else { k.allow = 0x1FFFu; k.wscale = 1.f; }
+    return k;
+}
 
 void launch_extrapolate(const float *x, const float *xm, float beta, float *y, size_t n, cudaStream_t st) {
     k_extrapolate<<<ew_blocks(n), 256, 0, st>>>(x, xm, beta, y, n); TC_COUNT_LAUNCH();
 }
-void launch_residual(const float *Ax, const float *Axm, const float *b, float beta, float *Ay, float *r, size_t n, cudaStream_t st) {
-    k_residual<<<ew_blocks(n), 256, 0, st>>>(Ax, Axm, b, beta, Ay, r, n); TC_COUNT_LAUNCH();
+void launch_residual(const float *Ax, const float *Axm, const float *b, float beta, float *r, size_t n, cudaStream_t st) {
+    k_residual<<<ew_blocks(n), 256, 0, st>>>(Ax, Axm, b, beta, r, n); TC_COUNT_LAUNCH();
 }
-void launch_update(const float *y, const float *atr, PriorDev pr, float invL, float *g, float *z, int S, int n, cudaStream_t st,
-                   int s_first, int n_out) {
+void launch_update(const float *x, const float *xm, float beta, const float *atr, PriorDev pr, float invL, float *g, float *z, int S, int n,
+                   cudaStream_t st, int s_first, int n_out) {
     if (n_out < 0) n_out = S - s_first;
     dim3 gr((n + 31) / 32, (n + 7) / 8, (n_out + PM_ZC - 1) / PM_ZC);
-    if (z) k_prior_grad_march<true><<<gr, PM_THREADS, 0, st>>>(y, atr, mk(pr), pr.lambda, invL, g, z, S, n, s_first, n_out);
-    else   k_prior_grad_march<false><<<gr, PM_THREADS, 0, st>>>(y, atr, mk(pr), pr.lambda, invL, g, nullptr, S, n, s_first, n_out);
+    const PriorK k = mk(pr);
+    if (xm) {
+        if (z) k_prior_grad_march<true, true><<<gr, PM_THREADS, 0, st>>>(x, xm, beta, atr, k, pr.lambda, invL, g, z, S, n, s_first, n_out);
+        else   k_prior_grad_march<false, true><<<gr, PM_THREADS, 0, st>>>(x, xm, beta, atr, k, pr.lambda, invL, g, nullptr, S, n, s_first, n_out);
+    } else {
+        if (z) k_prior_grad_march<true, false><<<gr, PM_THREADS, 0, st>>>(x, nullptr, 0.f, atr, k, pr.lambda, invL, g, z, S, n, s_first, n_out);
+        else   k_prior_grad_march<false, false><<<gr, PM_THREADS, 0, st>>>(x, nullptr, 0.f, atr, k, pr.lambda, invL, g, nullptr, S, n, s_first, n_out);
+    }
     TC_COUNT_LAUNCH();
 }
-void launch_candidate_sino(const float *Ay, const float *Ag, const float *b, float invL, float *Az, double *acc, size_t n, cudaStream_t st) {
-    k_candidate_sino<<<RED_BLOCKS, RED_THREADS, 0, st>>>(Ay, Ag, b, invL, Az, acc + 16, n); TC_COUNT_LAUNCH();
+void launch_step(const float *x, const float *xm, float beta, const float *g, float alpha, int nonneg, float *z, size_t n, cudaStream_t st) {
+    k_step<<<ew_blocks(n), 256, 0, st>>>(x, xm, beta, g, alpha, nonneg, z, n); TC_COUNT_LAUNCH();
+}
+void launch_candidate_sino(const float *A0, const float *A1, const float *Ag, const float *b, float beta, float alpha, float *Az, double *acc,
+                           size_t n, cudaStream_t st) {
+    k_candidate_sino<<<RED_BLOCKS, RED_THREADS, 0, st>>>(A0, A1, Ag, b, beta, alpha, Az, acc + 16, n); TC_COUNT_LAUNCH();
     final_reduce(acc, 0, 0.5, st);
 }
 void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, int n, cudaStream_t st, int S_own) {
     if (S_own < 0) S_own = S;
-    if (grad) { PriorDev p1 = pr; p1.lambda = 1.f; launch_update(z, nullptr, p1, 0.f, grad, nullptr, S, n, st); }
+    if (grad) { PriorDev p1 = pr; p1.lambda = 1.f; launch_update(z, nullptr, 0.f, nullptr, p1, 0.f, grad, nullptr, S, n, st); }
     if (acc) {
-        k_prior_value_march<<<RED_BLOCKS, PM_THREADS, 0, st>>>(z, mk(pr), acc + 16, S, n, S_own); TC_COUNT_LAUNCH();
+        k_prior_value_march<false><<<RED_BLOCKS, PM_THREADS, 0, st>>>(z, nullptr, 0.f, nullptr, mk(pr), acc + 16, S, n, S_own); TC_COUNT_LAUNCH();
         final_reduce(acc, 1, 1.0, st);
     }
+}
+void launch_prior_curvature(const float *x, const float *xm, float beta, const float *g, PriorDev pr, double *acc, int slot, int S, int n, cudaStream_t st) {
+    k_prior_value_march<true><<<RED_BLOCKS, PM_THREADS, 0, st>>>(x, xm, beta, g, mk(pr), acc + 16, S, n, S); TC_COUNT_LAUNCH();
+    final_reduce(acc, slot, 1.0, st);
 }
 void launch_sumsq(const float *v, size_t n, double *acc, int slot, cudaStream_t st) {
     k_sumsq<<<RED_BLOCKS, RED_THREADS, 0, st>>>(v, n, acc + 16); TC_COUNT_LAUNCH();

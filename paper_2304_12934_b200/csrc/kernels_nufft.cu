@@ -165,6 +165,6 @@ __global__ void TC_LB2 k_adj_rows(DevPlan d, const float2 *__restrict__ rowbuf, 
     }
 }
 
-#include "kernels_polar.inc"
+#include "kernels_polar.cuh"
 
 }  // namespace tc

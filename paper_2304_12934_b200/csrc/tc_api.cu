@@ -35,7 +35,7 @@ struct tc_plan {
     int max_slab;                 // slices per slab (multiple of 8), 0 = not yet decided
     // device tables
     float2 *twG = nullptr, *twD = nullptr, *ph_fwd = nullptr, *ph_adj = nullptr, *ph_fbp[2] = {nullptr, nullptr};
-    int fbp_filter = 0;
+    int fbp_filter = -1;          // >= 0 only while tc_fbp runs: index into ph_fbp
     float *deapod = nullptr, *th_sorted = nullptr;
     double2 *cs = nullptr, *cs_sorted = nullptr;
     int *a_sorted = nullptr, *tile_nr = nullptr;
@@ -54,20 +54,34 @@ struct tc_plan {
     cudaStream_t s_h2d = nullptr, s_comp = nullptr, s_d2h = nullptr;
     tc_sched_stats stats{};
     // per-stage CUDA-event timing (tc_profile)
-    bool prof = false;
+    bool prof = false, prof_open = false;
     struct ProfRec { int stage; cudaEvent_t a, b; };
     std::vector<ProfRec> prof_recs;
+    std::vector<cudaEvent_t> prof_pool;
 };
 
+// Events are pooled and reused (no cudaEventCreate inside a timed loop); at most PROF_MAX_RECS records are kept between two
+// tc_profile_read calls (a long tc_mbir run with profiling on then simply stops recording).
+constexpr size_t PROF_MAX_RECS = 1 << 16;
 static void prof_stage(tc_plan *p, int stage, cudaStream_t st, bool begin) {
     if (!p->prof) return;
     if (begin) {
+        p->prof_open = false;
+        if (p->prof_recs.size() >= PROF_MAX_RECS) return;
         tc_plan::ProfRec r; r.stage = stage;
-        cudaEventCreate(&r.a); cudaEventCreate(&r.b);
-        cudaEventRecord(r.a, st);
+        if (p->prof_pool.size() >= 2) {
+            r.a = p->prof_pool.back(); p->prof_pool.pop_back();
+            r.b = p->prof_pool.back(); p->prof_pool.pop_back();
+        } else if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) { cudaGetLastError(); return; }
+        if (cudaEventRecord(r.a, st) != cudaSuccess) { cudaGetLastError(); p->prof_pool.push_back(r.a); p->prof_pool.push_back(r.b); return; }
         p->prof_recs.push_back(r);
-    } else {
-        cudaEventRecord(p->prof_recs.back().b, st);
+        p->prof_open = true;
+    } else if (p->prof_open) {
+        if (cudaEventRecord(p->prof_recs.back().b, st) != cudaSuccess) {
+            cudaGetLastError();
+            p->prof_pool.push_back(p->prof_recs.back().a); p->prof_pool.push_back(p->prof_recs.back().b); p->prof_recs.pop_back();
+        }
+        p->prof_open = false;
     }
 }
 #define STAGE(id, call) do { prof_stage(p, id, st, true); call; prof_stage(p, id, st, false); } while (0)
@@ -283,6 +297,8 @@ extern "C" tc_status tc_plan_destroy(tc_plan *p) {
     if (p->d.side) cudaStreamDestroy(p->d.side);
     if (p->d.ev_fork) cudaEventDestroy(p->d.ev_fork);
     if (p->d.ev_join) cudaEventDestroy(p->d.ev_join);
+    for (auto &r : p->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (auto &e : p->prof_pool) cudaEventDestroy(e);
     if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
     if (p->s_comp) cudaStreamDestroy(p->s_comp);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
@@ -296,19 +312,21 @@ static size_t group_bytes(const tc_plan *p) {
     return ((size_t)d.G * d.G + (size_t)d.n * d.G + (size_t)d.na * d.nd) * P * sizeof(float2);
 }
 
-// Decide the slab size (slices per pass through the pipeline) and allocate scratch for it.
-static tc_status ensure_scratch(tc_plan *p, int n_slices, int *slab_out) {
+// Decide the slab size (slices per pass through the pipeline) and allocate scratch for it: at most `cap_groups` groups
+// (0 = no cap) and at most `frac` of the free device memory.  Scratch only ever grows; a smaller request reuses what is there.
+static tc_status ensure_scratch(tc_plan *p, int n_slices, int *slab_out, int cap_groups = 0, double frac = 0.45) {
     int want = (n_slices + 7) / 8;                                   // groups
     if (p->max_slab) want = std::min(want, p->max_slab / 8);
-    if (want <= p->ng_alloc) { *slab_out = p->ng_alloc * 8; return TC_OK; }
-    if (p->ng_alloc == 0 || want > p->ng_alloc) {
+    if (cap_groups > 0) want = std::min(want, cap_groups);
+    if (want > p->ng_alloc) {
         size_t fr = 0, tot = 0;
         CU(cudaMemGetInfo(&fr, &tot));
-        size_t have = (size_t)p->ng_alloc * group_bytes(p);
-        size_t budget = (size_t)((fr + have) * 0.45);
-        int fit = (int)std::max<size_t>(1, budget / group_bytes(p));
+        const size_t have = (size_t)p->ng_alloc * group_bytes(p);
+        const size_t budget = (size_t)((fr + have) * frac);
+        const int fit = (int)std::max<size_t>(1, budget / group_bytes(p));
         want = std::min(want, fit);
-        if (want <= p->ng_alloc) { *slab_out = p->ng_alloc * 8; return TC_OK; }
+    }
+    if (want > p->ng_alloc) {
         cudaFree(p->rowbuf); cudaFree(p->grid); cudaFree(p->cpol);
         p->rowbuf = p->grid = p->cpol = nullptr; p->ng_alloc = 0;
         const DevPlan &d = p->d;
@@ -328,19 +346,12 @@ static void forward_slab(tc_plan *p, const float *vol, int S, float *sino, cudaS
     STAGE(1, launch_fwd_cols(p->d, p->rowbuf, ng, p->grid, st));
     STAGE(2, launch_fwd_gather(p->d, p->grid, S, ng, sino, st));
 }
-// tc_fbp: the adjoint pipeline with the FBP-weighted phase table in place of ph_adj (one multiply in B1)
-static void fbp_slab(tc_plan *p, const float *sino, int S, float *vol, cudaStream_t st) {
-    const int ng = (S + 7) / 8;
-    DevPlan d2 = p->d;
-    d2.ph_adj = p->ph_fbp[p->fbp_filter];
-    STAGE(3, launch_adj_radial(d2, sino, S, ng, p->cpol, st));
-    STAGE(4, launch_adj_spread(p->d, p->cpol, ng, p->grid, st));
-    STAGE(5, launch_adj_cols(p->d, p->grid, ng, p->rowbuf, st));
-    STAGE(6, launch_adj_rows(p->d, p->rowbuf, S, ng, vol, st));
-}
+// B1-B4.  tc_fbp is the same pipeline with the FBP-weighted phase table in place of ph_adj (one multiply in B1): p->fbp_filter >= 0.
 static void adjoint_slab(tc_plan *p, const float *sino, int S, float *vol, cudaStream_t st) {
     const int ng = (S + 7) / 8;
-    STAGE(3, launch_adj_radial(p->d, sino, S, ng, p->cpol, st));
+    DevPlan d1 = p->d;
+    if (p->fbp_filter >= 0) d1.ph_adj = p->ph_fbp[p->fbp_filter];
+    STAGE(3, launch_adj_radial(d1, sino, S, ng, p->cpol, st));
     STAGE(4, launch_adj_spread(p->d, p->cpol, ng, p->grid, st));
     STAGE(5, launch_adj_cols(p->d, p->grid, ng, p->rowbuf, st));
     STAGE(6, launch_adj_rows(p->d, p->rowbuf, S, ng, vol, st));
@@ -359,7 +370,7 @@ extern "C" tc_status tc_profile_read(tc_plan *p, double *ms, long long *launches
         CU(cudaEventSynchronize(r.b));
         CU(cudaEventElapsedTime(&t, r.a, r.b));
         ms[r.stage] += t; launches[r.stage] += 1;
-        cudaEventDestroy(r.a); cudaEventDestroy(r.b);
+        p->prof_pool.push_back(r.a); p->prof_pool.push_back(r.b);
     }
     p->prof_recs.clear();
     return TC_OK;
@@ -377,5 +388,37 @@ static bool is_device_ptr(const void *ptr) {
     return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
 }
 
-#include "tc_api_part3.inc"
-#include "tc_api_part2.inc"
+// Owns device / pinned-host allocations and host registrations of one call: everything is released on every return path.
+struct CallMem {
+    std::vector<void *> dev, host, reg;
+    template <class T> cudaError_t alloc(T **ptr, size_t elems) {
+        cudaError_t e = cudaMalloc((void **)ptr, std::max<size_t>(elems, 1) * sizeof(T));
+        if (e == cudaSuccess) dev.push_back(*ptr); else { *ptr = nullptr; cudaGetLastError(); }
+        return e;
+    }
+    template <class T> cudaError_t alloc_host(T **ptr, size_t elems) {
+        cudaError_t e = cudaMallocHost((void **)ptr, std::max<size_t>(elems, 1) * sizeof(T));
+        if (e == cudaSuccess) host.push_back(*ptr); else { *ptr = nullptr; cudaGetLastError(); }
+        return e;
+    }
+    // page-locks caller memory for the duration of the call if it is pageable; returns true if the range is pinned afterwards
+    bool pin(const void *ptr, size_t bytes) {
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, ptr) != cudaSuccess) { cudaGetLastError(); return false; }
+        if (at.type == cudaMemoryTypeHost) return true;
+        if (at.type != cudaMemoryTypeUnregistered) return false;
+        if (cudaHostRegister(const_cast<void *>(ptr), bytes, cudaHostRegisterDefault) != cudaSuccess) { cudaGetLastError(); return false; }
+        reg.push_back(const_cast<void *>(ptr));
+        return true;
+    }
+    void release() {
+        for (void *q : dev) cudaFree(q);
+        for (void *q : host) cudaFreeHost(q);
+        for (void *q : reg) cudaHostUnregister(q);
+        dev.clear(); host.clear(); reg.clear();
+    }
+    ~CallMem() { release(); }
+};
+
+#include "tc_ops.cuh"
+#include "tc_mbir_streamed.cuh"

@@ -262,31 +262,41 @@ def test_mbir_host_pointers_and_default_L(tc):
         plan2.mbir(_cuda(b), tc.prior_params(0.9, SIG, C), 1)                 # p outside (1, 2]
 
 
-def test_full_size_config4_geometry_sampled(tc):
-    # BASELINE config 4 geometry (2048^2, 1024 angles, centre 1027.5) in the launch configuration bench.py times,
-    # 8 slices (one group; groups are independent CTAs).  Slice 5: full oracle NUFFT; two angles and a few pixels
-    # against the direct DFT.
+def test_full_size_config4_timed_launch_configuration(tc):
+    # BASELINE config 4 exactly as bench.py times it: 128 slices of 2048^2 (16 groups: k_adj_spread<4> looping four group blocks
+    # per thread, the <4> heavy-cell kernel on the side stream), 1024 angles, centre 1027.5.  Slices 5 and 101 (different group
+    # blocks) against the full oracle NUFFT, two angles and a few pixels against the direct DFT, adjoint identity over all 128.
     from paper_2304_12934_b200 import inputs
     from oracle import nufft, direct
+    from oracle_pool import OraclePool, n_workers
     c = inputs.CONFIGS[4]
+    S = c["S"]
     ang = inputs.angles_uniform(c["Na"]); a64 = ang.astype(np.float64)
-    vol = inputs.volume_fibres(8, c["N"], c["seed"], n_fibres=600)
+    vol = inputs.volume_fibres(S, c["N"], c["seed"], n_fibres=600, workers=n_workers())
     plan = tc.Plan(c["N"], c["Nd"], ang, c["centre"])
     s = _np(plan.radon(_cuda(vol)))
-    so = nufft.radon_nufft(vol[5], a64, c["Nd"], c["centre"])
-    assert rel_l2(s[5], so) < TOL_NUFFT
-    sel = [137, 700]
-    assert rel_l2(s[5][sel], direct.radon_direct(vol[5], a64[sel], c["Nd"], c["centre"])) < TOL_DIRECT
-    y = so.astype(np.float32)[None].repeat(8, axis=0); y[2] *= 0.5
-    b = _np(plan.backproject(_cuda(y)))
-    plan.close()
-    bo = nufft.backproject_nufft(y[5], a64, c["N"], c["centre"])
-    assert rel_l2(b[5], bo) < TOL_NUFFT and rel_l2(b[2], 0.5 * bo) < TOL_NUFFT
-    rng = np.random.default_rng(17)
-    yr = rng.standard_normal((8, c["Na"], c["Nd"])).astype(np.float32)
-    plan = tc.Plan(c["N"], c["Nd"], ang, c["centre"])
-    br = _np(plan.backproject(_cuda(yr))); plan.close()
-    assert _adj_mismatch(vol, yr, s, br) < TOL_ADJ
+    pick = [5, 101]
+    with OraclePool(a64, c["N"], c["Nd"], c["centre"]) as op:
+        so = op.A(vol[pick])
+        for k, sl in enumerate(pick):
+            assert rel_l2(s[sl], so[k]) < TOL_NUFFT
+        sel = [137, 700]
+        assert rel_l2(s[101][sel], direct.radon_direct(vol[101], a64[sel], c["Nd"], c["centre"])) < TOL_DIRECT
+        rng = np.random.default_rng(17)
+        y = rng.standard_normal((S, c["Na"], c["Nd"])).astype(np.float32)
+        y[5] = so[0]; y[101] = 0.5 * so[1]
+        b = _np(plan.backproject(_cuda(y)))
+        plan.close()
+        bo = op.At(y[pick].astype(np.float64))
+    for k, sl in enumerate(pick):
+        assert rel_l2(b[sl], bo[k]) < TOL_NUFFT
+    x = np.arange(c["N"]) - c["N"] // 2                                   # two pixels of slice 101 against the definition (D2),
+    u = np.arange(c["Nd"])                                                # evaluated through its Dirichlet-kernel closed form
+    for (i, j) in ((1000, 1100), (317, 1500)):
+        t = x[j] * np.cos(a64)[:, None] + x[i] * np.sin(a64)[:, None]
+        want = np.sum(y[101].astype(np.float64) * direct.dirichlet(u[None, :] - c["centre"] - t, c["Nd"]))
+        assert abs(b[101][i, j] - want) < TOL_DIRECT * np.sqrt(np.mean(b[101].astype(np.float64) ** 2))
+    assert _adj_mismatch(vol, y, s, b) < TOL_ADJ
 
 
 def test_mbir_out_of_core_streaming_matches_in_core_and_oracle(tc):
@@ -367,3 +377,236 @@ def test_fbp_vs_oracle(tc):
     rec = _np(plan.fbp(plan.radon(_cuda(vol))))
     plan.close()
     assert rel_l2(rec, vol) < 0.15                                   # sharp-edged ellipses, band-limited reconstruction
+
+
+# ---- M5 reject / restart on the GPU, in core and streamed (never executed by a test) -----------------------------
+import functools
+
+
+@functools.lru_cache(maxsize=None)
+def _reject_case(name):
+    """cases whose oracle run rejects candidates (replayed in tests/test_oracle_pins.py style probes; decisions have margins
+    >= 2.5e-4, far above the float32 noise of F).  Returns (b, ang, n, centre, (p, sigma, c, lam), L, iters, xo, logo, its)."""
+    from paper_2304_12934_b200 import inputs
+    from oracle import nufft, mbir
+    if name == "quadratic":            # p = 2, strong prior: momentum overshoots once (iteration 25) -- single rejection late in the run
+        n, na, S, centre, iters = 32, 16, 11, 16.0, 32
+        ang = (np.arange(na) * math.pi / na).astype(np.float32); a64 = ang.astype(np.float64)
+        truth = np.zeros((S, n, n)); truth[:, 10:22, 8:20] = 1.0; truth[1::2, 14:18, 12:26] += 0.5
+        truth += 0.05 * np.arange(S)[:, None, None] * (np.arange(n)[None, :, None] > 16)
+        b = (nufft.radon_nufft(truth, a64, n, centre) + 0.01 * np.random.default_rng(35).standard_normal((S, na, n))).astype(np.float32)
+        pr = (2.0, 1.0, 1.0, 200.0)
+        L, _ = mbir.lipschitz(n, a64, n, centre, *pr)
+    else:                              # the paper's prior with a step that is too long: L = cf * lambda_hat
+        S, n, na, centre = 10, 64, 24, 32.0
+        ang = inputs.angles_uniform(na); a64 = ang.astype(np.float64)
+        b = (nufft.radon_nufft(inputs.volume_cfg2(S=S, n=n), a64, n, centre)
+             + 0.01 * np.random.default_rng(18).standard_normal((S, na, n))).astype(np.float32)
+        pr = (P, SIG, C, 1.0)
+        _, lam_hat = mbir.lipschitz(n, a64, n, centre, *pr)
+        cf, iters = {"alternating": (0.6, 14), "stuck": (0.48, 6)}[name]
+        L = cf * lam_hat
+    xo, logo, its = mbir.mbir(b, a64, n, centre, *pr, L, iters, keep_iterates=True)
+    return b, ang, n, centre, pr, float(L), iters, xo, logo, its
+
+
+@pytest.mark.parametrize("name,pattern", [
+    ("alternating", [1, 0, 1, 0, 1, 0, 1, 0, 1, 0, 1, 1, 0, 1]),     # reject, plain step, momentum step, reject, ...
+    ("stuck", [1, 0, 0, 0, 0, 0]),                                   # consecutive rejections: the iterate must stand still
+    ("quadratic", None),
+])
+@pytest.mark.parametrize("streamed", [False, True])
+def test_mbir_reject_restart_in_core_and_streamed(tc, name, pattern, streamed):
+    b, ang, n, centre, pr, L, iters, xo, logo, its = _reject_case(name)
+    acc_o = [l["accepted"] for l in logo]
+    assert 0 in acc_o and (pattern is None or acc_o == pattern)
+    if name == "quadratic":
+        assert acc_o.index(0) == 25
+    prior = tc.prior_params(*pr, L)
+    if streamed:                                                      # 10 / 11 slices in slabs of 8: halos and the host-side buffer rotation
+        plan = tc.Plan(n, b.shape[-1], ang, centre, max_slab_slices=8)
+        x, log = plan.mbir(b, prior, iters)
+        assert plan.sched_stats()["n_slabs"] == 2
+    else:
+        plan = tc.Plan(n, b.shape[-1], ang, centre)
+        x, log = plan.mbir(_cuda(b), prior, iters)
+        x = _np(x)
+    plan.close()
+    assert [l["accepted"] for l in log] == acc_o
+    assert rel_l2(x, xo) < TOL_MBIR
+    for lg, lo in zip(log, logo):
+        assert abs(lg["F"] - lo["F"]) < 1e-4 * abs(lo["F"]) and abs(lg["beta"] - lo["beta"]) < 1e-6
+        assert abs(lg["margin"] - lo["margin"]) < 1e-4 + 1e-3 * abs(lo["margin"])
+    for k in range(iters):                                            # the step after a rejection is a plain gradient step
+        if not acc_o[k] and k + 1 < iters:
+            assert log[k + 1]["beta"] == 0.0
+    if not streamed:                                                  # the kept iterate is bit-identical across a rejected step
+        k = acc_o.index(0)
+        plan = tc.Plan(n, b.shape[-1], ang, centre)
+        xa = _np(plan.mbir(_cuda(b), prior, k)[0]); xb = _np(plan.mbir(_cuda(b), prior, k + 1)[0])
+        plan.close()
+        assert np.array_equal(xa, xb) and rel_l2(xb, its[k]) < TOL_MBIR
+
+
+def test_mbir_config1_iterate_by_iterate(tc):
+    # north_star: "MBIR iterates must match the oracle iterate-by-iterate": tc_mbir with iters = 1 .. 10 against the oracle's k-th iterate
+    from paper_2304_12934_b200 import inputs
+    from oracle import nufft, mbir
+    c = inputs.CONFIGS[1]
+    ang = inputs.angles_uniform(c["Na"]); a64 = ang.astype(np.float64)
+    b = nufft.radon_nufft(inputs.volume_cfg1(), a64, c["Nd"], c["centre"]).astype(np.float32)
+    L, _ = mbir.lipschitz(c["N"], a64, c["Nd"], c["centre"], P, SIG, C, 1.0)
+    xo, logo, its = mbir.mbir(b, a64, c["N"], c["centre"], P, SIG, C, 1.0, L, 10, keep_iterates=True)
+    plan = tc.Plan(c["N"], c["Nd"], ang, c["centre"])
+    worst = 0.0
+    for k in range(1, 11):
+        x, log = plan.mbir(_cuda(b), tc.prior_params(P, SIG, C, 1.0, L), k)
+        worst = max(worst, rel_l2(_np(x), its[k - 1]))
+        assert abs(log[-1]["F"] - logo[k - 1]["F"]) < 1e-4 * logo[k - 1]["F"]
+    plan.close()
+    assert worst < TOL_MBIR
+
+
+# ---- MBIR parity at the sizes of the BASELINE configs (VERDICT r1: parity stopped at 64^2) ---------------------------------
+def _mbir_full_size(tc, b, ang, n, nd, centre, L, iters, **plan_kw):
+    """oracle (operators over the process pool of tests/oracle_pool.py) vs tc_mbir; returns (x_gpu, log_gpu, x_oracle, log_oracle)."""
+    from oracle import mbir
+    from oracle_pool import OraclePool
+    a64 = ang.astype(np.float64)
+    with OraclePool(a64, n, nd, centre) as op, op.patched(mbir):
+        xo, logo = mbir.mbir(b, a64, n, centre, P, SIG, C, 1.0, L, iters)
+    plan = tc.Plan(n, nd, ang, centre, **plan_kw)
+    host = bool(plan_kw)
+    x, log = plan.mbir(b if host else _cuda(b), tc.prior_params(P, SIG, C, 1.0, L), iters)
+    x = x if host else _np(x)
+    plan.close()
+    assert [l["accepted"] for l in log] == [l["accepted"] for l in logo]
+    assert rel_l2(x, xo) < TOL_MBIR
+    for lg, lo in zip(log, logo):
+        assert abs(lg["F"] - lo["F"]) < 1e-4 * abs(lo["F"])
+    return x, log, xo, logo
+
+
+def test_mbir_config2_in_full(tc):
+    # BASELINE config 2: 16 slices of 256^2, 181 angles, 20 MBIR iterations (two groups; PM_ZC = 16 is exactly one chunk)
+    from paper_2304_12934_b200 import inputs
+    from oracle_pool import OraclePool
+    c = inputs.CONFIGS[2]
+    ang = inputs.angles_uniform(c["Na"])
+    with OraclePool(ang, c["N"], c["Nd"], c["centre"]) as op:
+        b = op.A(inputs.volume_cfg2()).astype(np.float32)
+    L = 1.05 * 1.02 * c["Na"] * c["N"] + 4.0 / (C * SIG * SIG)          # the same number goes to both sides (G15 is tested elsewhere)
+    x, log, xo, logo = _mbir_full_size(tc, b, ang, c["N"], c["Nd"], c["centre"], L, 20)
+    F = [l["F"] for l in log]
+    assert all(F[i + 1] <= F[i] for i in range(len(F) - 1))
+
+
+def test_mbir_config3_geometry(tc):
+    # BASELINE config 3 geometry (1024^2, 128 sparse angles, Poisson noise at 1e4 photons per bin), 4 slices, 10 iterations:
+    # the compile-time pass list 16,16,4 and the prior kernels' 32 x 8 tiling over 32 x 128 tiles
+    from paper_2304_12934_b200 import inputs
+    from oracle_pool import OraclePool
+    c = inputs.CONFIGS[3]
+    ang = inputs.angles_uniform(c["Na"])
+    with OraclePool(ang, c["N"], c["Nd"], c["centre"]) as op:
+        clean = op.A(inputs.volume_porous(4, c["N"], c["seed"]))
+    b = inputs.poisson_sinogram(clean, seed=19)
+    L = 1.05 * 1.02 * c["Na"] * c["N"] + 4.0 / (C * SIG * SIG)
+    _mbir_full_size(tc, b, ang, c["N"], c["Nd"], c["centre"], L, 10)
+
+
+def test_mbir_config5_geometry(tc):
+    # BASELINE config 5 geometry (2560^2 = 2^9 * 5: radix-5 pass lists, 1313 angles), 2 slices, 3 iterations, host pointers
+    # (the library decides: fits, so in core); then the same geometry streamed in forced 8-slice slabs against the in-core run
+    from paper_2304_12934_b200 import inputs
+    from oracle_pool import OraclePool, n_workers
+    c = inputs.CONFIGS[5]
+    ang = inputs.angles_uniform(c["Na"])
+    vol = inputs.volume_fibres(10, c["N"], c["seed"], n_fibres=400, workers=n_workers())
+    with OraclePool(ang, c["N"], c["Nd"], c["centre"]) as op:
+        b2 = op.A(vol[:2]).astype(np.float32)
+    L = 1.05 * 1.02 * c["Na"] * c["N"] + 4.0 / (C * SIG * SIG)
+    _mbir_full_size(tc, b2, ang, c["N"], c["Nd"], c["centre"], L, 3)
+    plan = tc.Plan(c["N"], c["Nd"], ang, c["centre"])
+    b10 = _np(plan.radon(_cuda(vol)))                                  # GPU-vs-GPU consistency only from here on
+    pr = tc.prior_params(P, SIG, C, 1.0, L)
+    x_in, log_in = plan.mbir(_cuda(b10), pr, 3); x_in = _np(x_in)
+    plan.close()
+    plan = tc.Plan(c["N"], c["Nd"], ang, c["centre"], max_slab_slices=8)
+    x_st, log_st = plan.mbir(b10, pr, 3)
+    assert plan.sched_stats()["n_slabs"] == 2
+    plan.close()
+    assert rel_l2(x_st, x_in) <= 1e-5 and [l["accepted"] for l in log_st] == [l["accepted"] for l in log_in]
+    for ls, li in zip(log_st, log_in):
+        assert abs(ls["F"] - li["F"]) <= 1e-6 * abs(li["F"])
+
+
+# ---- SURVEY 8(f): neighbour sets (row 4), majorise-minimise step length (row 1) ------------------------------------------
+def test_prior_neighbour_sets_vs_oracle(tc):
+    from oracle import prior
+    rng = np.random.default_rng(40)
+    v = (rng.standard_normal((19, 40, 70)) * 0.3).astype(np.float32)      # two z-chunks of the march kernels, ragged tiles
+    for nb in (26, 10, 6):
+        val, g = tc.prior_eval(_cuda(np.ascontiguousarray(v[:, :, :40])), tc.prior_params(P, SIG, C, neighbours=nb))
+        vo = v[:, :, :40]
+        assert abs(val - prior.H(vo, P, SIG, C, nb)) <= 2e-6 * prior.H(vo, P, SIG, C, nb)
+        assert rel_l2(_np(g), prior.gradH(vo, P, SIG, C, nb)) < 1e-5
+    with pytest.raises(tc.TcError):
+        tc.prior_eval(_cuda(v[:, :40, :40].copy()), tc.prior_params(P, SIG, C, neighbours=18))
+
+
+@pytest.mark.parametrize("kw", [dict(neighbours=10), dict(mm_step=True), dict(mm_step=True, neighbours=6, nonneg=True)])
+def test_mbir_variants_vs_oracle(tc, kw):
+    # 11 slices of 64^2 (two groups), noisy data; the variant's flag goes to both sides; alpha is compared where it is logged
+    from paper_2304_12934_b200 import inputs
+    from oracle import nufft, mbir
+    S, n, na, centre, iters = 11, 64, 24, 32.0, 8
+    ang = inputs.angles_uniform(na); a64 = ang.astype(np.float64)
+    b = (nufft.radon_nufft(inputs.volume_cfg2(S=S, n=n) - (0.25 if kw.get("nonneg") else 0.0), a64, n, centre)
+         + 0.02 * np.random.default_rng(41).standard_normal((S, na, n))).astype(np.float32)
+    L, _ = mbir.lipschitz(n, a64, n, centre, P, SIG, C, 1.0)
+    xo, logo = mbir.mbir(b, a64, n, centre, P, SIG, C, 1.0, L, iters, **kw)
+    plan = tc.Plan(n, n, ang, centre)
+    x, log = plan.mbir(_cuda(b), tc.prior_params(P, SIG, C, 1.0, L, **kw), iters)
+    x = _np(x); plan.close()
+    assert [l["accepted"] for l in log] == [l["accepted"] for l in logo]
+    assert rel_l2(x, xo) < TOL_MBIR
+    for lg, lo in zip(log, logo):
+        assert abs(lg["F"] - lo["F"]) < 1e-4 * abs(lo["F"])
+        assert abs(lg["alpha"] - lo["alpha"]) < 1e-4 * lo["alpha"]
+    if kw.get("mm_step"):
+        assert max(l["alpha"] for l in logo) > 1.5 / L                    # the MM step is longer than the fixed one: the flag acts
+        plan = tc.Plan(n, n, ang, centre, max_slab_slices=8)
+        with pytest.raises(tc.TcError) as e:                              # streamed problems: documented TC_EUNSUPPORTED
+            plan.mbir(b, tc.prior_params(P, SIG, C, 1.0, L, **kw), 2)
+        assert e.value.status == tc.TC_EUNSUPPORTED
+        plan.close()
+
+
+def test_error_paths_release_device_memory(tc):
+    # tc.h: the plan owns all scratch, a failed call leaves nothing behind.  A working set that cannot fit (device pointers:
+    # TC_ENOMEM before any kernel runs), then a bad prior; free device memory is the same before and after.
+    import torch
+    ang = (np.arange(8) * math.pi / 8).astype(np.float32)
+    torch.cuda.synchronize(); torch.cuda.empty_cache()
+    free0 = torch.cuda.mem_get_info()[0]
+    plan = tc.Plan(1024, 1024, ang, 512.0)
+    tiny = torch.zeros((1, 8, 1024), dtype=torch.float32, device="cuda")
+    out = torch.zeros((1, 1024, 1024), dtype=torch.float32, device="cuda")
+    log = (tc.tc_iter_log * 1)()
+    pr = tc.prior_params(P, SIG, C, 1.0, 1e5)
+    import ctypes
+    st = tc.lib.tc_mbir(plan._h, tiny.data_ptr(), 60000, ctypes.byref(pr), 1, out.data_ptr(), log, None)     # 4 x 240 GB of state
+    assert st == tc.TC_ENOMEM and b"does not fit" in tc.lib.tc_last_error()
+    bad = tc.prior_params(0.5, SIG, C)
+    val = ctypes.c_double()
+    assert tc.lib.tc_prior_eval(out.data_ptr(), 1, 1024, ctypes.byref(bad), None, ctypes.byref(val)) == tc.TC_EINVAL
+    host = np.zeros((1, 64, 64), np.float32)
+    assert tc.lib.tc_prior_eval(host.ctypes.data, 1, 64, ctypes.byref(pr), out.data_ptr(), ctypes.byref(val)) == tc.TC_EINVAL   # mixed host / device
+    x, _ = plan.mbir(tiny, pr, 1)                                          # and the plan still works afterwards
+    torch.cuda.synchronize()
+    plan.close()
+    del tiny, out, x
+    torch.cuda.empty_cache()
+    free1 = torch.cuda.mem_get_info()[0]
+    assert abs(free1 - free0) <= 64 << 20, (free0, free1)

@@ -303,3 +303,198 @@ def test_fbp_nufft_matches_definition_and_weights():
     import unittest.mock as mock
     with mock.patch.object(fbp, "ramp_weights", lambda nd_, na_, window="ramp": np.ones(nd_ - 1)):
         assert rel_l2(fbp.fbp_direct(y, ang, n, 23.5), direct.backproject_direct(y, ang, n, 23.5)) < 1e-12
+
+
+# ---- the reject / restart branch of the optimiser ("monotonic ... with restart"; G14) -------------
+def _dense_case(cf):
+    N, na = 8, 10
+    ang = np.arange(na) * math.pi / na
+    b = np.random.default_rng(10).standard_normal((1, na, N))
+    An = np.stack([nufft.radon_nufft(e.reshape(N, N), ang, N, 4.0).ravel() for e in np.eye(N * N)], axis=1)
+    L = cf * np.linalg.norm(An, 2) ** 2
+    return An, b, ang, N, L
+
+
+def test_mbir_reject_restart_branch_from_dense_matrix():
+    # lambda = 0 on the brute-force 8 x 8 system with a step that is too long for the momentum (L = 0.6 ||A||^2): candidates are
+    # rejected.  Everything expected below is computed from the dense matrix and the textbook momentum numbers, not from mbir.py:
+    #   - a rejected step leaves the iterate bit-identical and F unchanged (monotone: "x- <- x", nothing else moves);
+    #   - the step after a rejection has beta = 0 and its candidate is the plain gradient step x - A^T (A x - b)/L from the
+    #     KEPT x (dropping `t = 1` fails the beta checks; dropping `xm = x` fails the second-step check, because the momentum
+    #     would then extrapolate from the older iterate);
+    #   - the step after that uses beta = (t1 - 1)/t2 = 0.28175..., t1 = (1 + sqrt 5)/2, on (x_{k+1}, x_k).
+    An, b, ang, N, L = _dense_case(0.6)
+    bv = b.ravel()
+    x, log, its = mbir.mbir(b, ang, N, 4.0, P, SIG, C, 0.0, L, 12, keep_iterates=True)
+    acc = [l["accepted"] for l in log]
+    assert acc[:7] == [1, 1, 1, 0, 1, 1, 0]
+    F = lambda v: 0.5 * np.sum((An @ v - bv) ** 2)
+    step = lambda y: y - An.T @ (An @ y - bv) / L
+    t1 = (1 + math.sqrt(5)) / 2; t2 = (1 + math.sqrt(1 + 4 * t1 * t1)) / 2
+    beta1 = (t1 - 1) / t2
+    assert abs(beta1 - 0.2817535) < 1e-6
+    for k in (3, 6):
+        assert np.array_equal(its[k], its[k - 1]) and log[k]["F"] == log[k - 1]["F"]            # rejected: nothing moved
+        # the rejected candidate was the momentum step from (x_{k-1}, x_{k-2}) and it did increase F
+        yk = its[k - 1].ravel() + log[k]["beta"] * (its[k - 1].ravel() - its[k - 2].ravel())
+        assert abs(log[k]["data"] - F(step(yk))) < 1e-10 * log[k]["data"] and log[k]["data"] > log[k - 1]["F"]
+        assert log[k]["margin"] < 0 and log[k]["beta"] > 0
+        assert log[k + 1]["beta"] == 0.0 and log[k + 1]["accepted"] == 1                         # restart: plain gradient step from the kept x
+        assert rel_l2(its[k + 1].ravel(), step(its[k].ravel())) < 1e-12
+        if k + 2 < len(log):
+            assert abs(log[k + 2]["beta"] - beta1) < 1e-15
+            y2 = its[k + 1].ravel() + beta1 * (its[k + 1].ravel() - its[k].ravel())              # x- is the kept iterate, not an older one
+            assert rel_l2(its[k + 2].ravel(), step(y2)) < 1e-12
+    # the momentum sequence restarts from scratch: betas after the restart repeat the betas from the start
+    assert [l["beta"] for l in log[4:6]] == [l["beta"] for l in log[0:2]]
+    for k, l in enumerate(log):                                                                  # logged F is the dense objective of the kept iterate
+        assert abs(l["F"] - F(its[k].ravel())) < 1e-10 * l["F"]
+
+
+def test_mbir_consecutive_rejections_keep_the_iterate():
+    # L = 0.45 ||A||^2: after two accepted steps even the plain gradient step increases F, so every later candidate is rejected;
+    # the loop must then stand still (same iterate, same F, beta = 0, the same rejected candidate every time).
+    An, b, ang, N, L = _dense_case(0.45)
+    bv = b.ravel()
+    x, log, its = mbir.mbir(b, ang, N, 4.0, P, SIG, C, 0.0, L, 9, keep_iterates=True)
+    assert [l["accepted"] for l in log] == [1, 0, 1, 0, 0, 0, 0, 0, 0]
+    cand = its[2].ravel() - An.T @ (An @ its[2].ravel() - bv) / L
+    Fc = 0.5 * np.sum((An @ cand - bv) ** 2)
+    for k in range(4, 9):
+        assert np.array_equal(its[k], its[2]) and log[k]["F"] == log[2]["F"] and log[k]["beta"] == 0.0
+        assert abs(log[k]["data"] - Fc) < 1e-10 * Fc and Fc > log[2]["F"]
+    assert np.array_equal(x, its[2])
+
+
+def test_lipschitz_power_iteration_vs_dense_norm():
+    # lambda_hat (10 power iterations from ones, reading G15) against the spectral norm of the brute-force matrix
+    An, b, ang, N, _ = _dense_case(1.0)
+    Lq, lam_hat = mbir.lipschitz(N, ang, N, 4.0, P, SIG, C, 0.0)
+    s2 = np.linalg.norm(An, 2) ** 2
+    assert 0.97 * s2 < lam_hat <= s2 * (1 + 1e-12) and abs(Lq - 1.05 * lam_hat) < 1e-12 * Lq
+    Lp, _ = mbir.lipschitz(N, ang, N, 4.0, P, SIG, C, 3.0)
+    assert abs(Lp - (1.05 * lam_hat + 3.0 * 4.0 / (C * SIG * SIG))) < 1e-9 * Lp                  # curvature bound h''(0) = 2/(c sigma^2), pairs double it
+
+
+def test_fbp_hann_window_read_off_a_single_radial_mode():
+    # A sinogram that is one radial mode, p[a][u] = cos(2 pi m0 (u - centre)/Nd), has coefficients at m = +-m0 only, so FBP of it
+    # is the plain adjoint (D2) times (pi/Na) (m0/Nd) win(m0): the filter value is read off exactly.  Hann = cos^2(pi m/Nd):
+    # 1, 3/4, 1/2, 1/4 at m0 = 0, Nd/6, Nd/4, Nd/3.
+    from oracle import fbp
+    n, nd, na, centre = 16, 48, 7, 23.25
+    ang = np.sort(np.random.default_rng(36).uniform(0, np.pi, na))
+    u = np.arange(nd)
+    for m0, win in ((8, 0.75), (12, 0.5), (16, 0.25), (3, math.cos(math.pi * 3 / 48) ** 2)):
+        p = np.tile(np.cos(2 * np.pi * m0 * (u - centre) / nd), (na, 1))
+        plain = direct.backproject_direct(p, ang, n, centre)
+        ramp = fbp.fbp_direct(p, ang, n, centre, "ramp")
+        hann = fbp.fbp_direct(p, ang, n, centre, "hann")
+        assert rel_l2(ramp, plain * (np.pi / na) * (m0 / nd)) < 1e-12
+        assert rel_l2(hann, ramp * win) < 1e-12
+        assert rel_l2(fbp.fbp_nufft(p, ang, n, centre, "hann"), hann) < 2e-5
+    p0 = np.ones((na, nd))                                          # m0 = 0: DC bin, weight 1/(4 Nd), Hann = 1
+    assert rel_l2(fbp.fbp_direct(p0, ang, n, centre, "hann"), direct.backproject_direct(p0, ang, n, centre) * (np.pi / na) * 0.25 / nd) < 1e-12
+
+
+def test_oracle_pool_is_scheduling_only():
+    # tests/oracle_pool.py (used by the full-size GPU parity tests) must return what the serial oracle returns
+    from oracle_pool import OraclePool
+    rng = np.random.default_rng(37); n, nd, na = 16, 24, 7
+    ang = rng.uniform(0, np.pi, na)
+    f = rng.standard_normal((3, n, n)); y = rng.standard_normal((3, na, nd))
+    b = nufft.radon_nufft(f, ang, nd, 11.5)
+    with OraclePool(ang, n, nd, 11.5, workers=2, chunks_per_slice=3) as op:
+        assert rel_l2(op.A(f), b) < 1e-14
+        assert rel_l2(op.At(y), nufft.backproject_nufft(y, ang, n, 11.5)) < 1e-13
+        x0, log0 = mbir.mbir(b, ang, n, 11.5, P, SIG, C, 1.0, 500.0, 3)
+        with op.patched(mbir):
+            x1, log1 = mbir.mbir(b, ang, n, 11.5, P, SIG, C, 1.0, 500.0, 3)
+        assert rel_l2(x1, x0) < 1e-12 and [l["accepted"] for l in log1] == [l["accepted"] for l in log0]
+    assert mbir.nufft.radon_nufft is nufft.radon_nufft
+
+
+# ---- neighbour sets; row 1: majorise-minimise step length ------------------------------------------
+@pytest.mark.parametrize("nb,wsum", [(10, 6 + 4 / math.sqrt(2)), (6, 6.0)])
+def test_prior_neighbour_sets_bruteforce(nb, wsum):
+    # 10 = the 8 in-plane neighbours and the 2 along z (the set P:L149 quotes for SVMBIR), 6 = faces; weights 1/distance / their sum
+    offs = prior.offsets(nb)
+    assert len(offs) == nb and abs(sum(prior.weight(o, nb) for o in offs) - 1.0) < 1e-14
+    rng = np.random.default_rng(38); f = rng.standard_normal((3, 4, 5))
+    idx = [(z, y, x) for z in range(3) for y in range(4) for x in range(5)]
+    tot = 0.0; grad = np.zeros_like(f)
+    for a in idx:
+        for b in idx:
+            dz, dy, dx = (abs(a[k] - b[k]) for k in range(3))
+            if max(dz, dy, dx) != 1 or not a < b:
+                continue
+            member = (dz == 0 or (dy == 0 and dx == 0)) if nb == 10 else (dz + dy + dx == 1)
+            if not member:
+                continue
+            w = 1 / math.sqrt(dz + dy + dx) / wsum
+            D = f[a] - f[b]; u = abs(D) / SIG; uq = u ** (2 - P)
+            tot += w * u * u / (C + uq)
+            d = w * math.copysign(1.0, D) / SIG * u * (2 * C + P * uq) / (C + uq) ** 2
+            grad[a] += d; grad[b] -= d
+    assert abs(prior.H(f, P, SIG, C, nb) - tot) < 1e-12 * tot
+    assert rel_l2(prior.gradH(f, P, SIG, C, nb), grad) < 1e-12
+    assert prior.H(f, P, SIG, C, 26) == prior.H(f, P, SIG, C)        # the default is untouched
+
+
+def test_prior_surrogate_curvature_majorises():
+    # curvH is the curvature of the symmetric-bound quadratic surrogate: Q(a) = H(f) - a <grad H(f), g> + a^2/2 curvH(f; g) >= H(f - a g)
+    # for 1 < p <= 2, touching at a = 0; for the quadratic case p = 2 (h = u^2 / (c + 1)) the surrogate IS the function.
+    rng = np.random.default_rng(39)
+    f = rng.standard_normal((3, 5, 6)); g = rng.standard_normal((3, 5, 6))
+    for nb in (26, 10):
+        H0, gr, cv = prior.H(f, P, SIG, C, nb), prior.gradH(f, P, SIG, C, nb), prior.curvH(f, g, P, SIG, C, nb)
+        for a in (1e-3, 0.05, 0.3, 1.0, 4.0, -0.7):
+            Q = H0 - a * np.sum(gr * g) + 0.5 * a * a * cv
+            assert prior.H(f - a * g, P, SIG, C, nb) <= Q * (1 + 1e-12)
+        a = 1e-4                                                      # tangent at a = 0: 0 <= Q - H <= a^2/2 curvH (a wrong slope would leave O(a))
+        gap = H0 - a * np.sum(gr * g) + 0.5 * a * a * cv - prior.H(f - a * g, P, SIG, C, nb)
+        assert -1e-13 <= gap <= 0.5 * a * a * cv
+    H0, gr, cv = prior.H(f, 2.0, 1.3, 0.5), prior.gradH(f, 2.0, 1.3, 0.5), prior.curvH(f, g, 2.0, 1.3, 0.5)
+    for a in (0.3, -2.0):
+        assert abs(H0 - a * np.sum(gr * g) + 0.5 * a * a * cv - prior.H(f - a * g, 2.0, 1.3, 0.5)) < 1e-12 * H0
+    assert abs(prior.dh_over_D(0.0, P, SIG, C) - 2.0 / (C * SIG * SIG)) < 1e-9 / (C * SIG * SIG)
+
+
+def test_mbir_mm_step_is_the_exact_line_minimiser_for_lambda0():
+    # lambda = 0: the majorise-minimise step is alpha = ||g||^2 / ||A g||^2, the exact minimiser of the quadratic along -g.
+    # From the brute-force matrix: the first iterate is steepest descent's x1 = alpha0 A^T b, and at every accepted step the new
+    # residual is orthogonal to A g (d/d alpha = 0).
+    An, b, ang, N, L = _dense_case(1.0)
+    bv = b.ravel()
+    x, log, its = mbir.mbir(b, ang, N, 4.0, P, SIG, C, 0.0, L, 6, keep_iterates=True, mm_step=True)
+    g0 = An.T @ (-bv)
+    a0 = np.sum(g0 * g0) / np.sum((An @ g0) ** 2)
+    assert abs(log[0]["alpha"] - a0) < 1e-12 * a0 and rel_l2(its[0].ravel(), -a0 * g0) < 1e-12
+    xk, xkm = np.zeros(N * N), np.zeros(N * N)
+    for k, l in enumerate(log):
+        y = xk + l["beta"] * (xk - xkm)
+        g = An.T @ (An @ y - bv)
+        z = y - l["alpha"] * g
+        assert abs(np.dot(An @ g, An @ z - bv)) < 1e-9 * np.linalg.norm(An @ g) * np.linalg.norm(An @ z - bv)
+        if l["accepted"]:
+            assert rel_l2(its[k].ravel(), z) < 1e-12
+            xkm, xk = xk, z
+    F = [l["F"] for l in log]
+    assert all(F[i + 1] <= F[i] for i in range(len(F) - 1))
+
+
+def test_mbir_mm_step_decreases_the_surrogate_with_prior():
+    # lambda > 0, first step (y = x = 0): F(z) <= Q(alpha*) = F(0) - ||g||^4 / (2 den) < F(0), den = ||A g||^2 + lam curvH(0; g),
+    # all evaluated here from the dense matrix and the (separately pinned) prior functions
+    An, b, ang, N, L = _dense_case(1.0)
+    bv = b.ravel(); lam = 0.7
+    x, log = mbir.mbir(b, ang, N, 4.0, P, SIG, C, lam, L, 8, mm_step=True, neighbours=10)
+    g = (An.T @ (-bv)).reshape(1, N, N)
+    den = np.sum((An @ g.ravel()) ** 2) + lam * prior.curvH(np.zeros((1, N, N)), g, P, SIG, C, 10)
+    a = np.sum(g * g) / den
+    assert abs(log[0]["alpha"] - a) < 1e-12 * a
+    F0 = 0.5 * np.sum(bv * bv)
+    z = -a * g
+    Fz = 0.5 * np.sum((An @ z.ravel() - bv) ** 2) + lam * prior.H(z, P, SIG, C, 10)
+    assert abs(log[0]["F"] - Fz) < 1e-10 * Fz and Fz <= F0 - 0.5 * np.sum(g * g) ** 2 / den + 1e-9 * F0
+    F = [l["F"] for l in log]
+    assert all(F[i + 1] <= F[i] for i in range(len(F) - 1)) and all(l["alpha"] > 0 for l in log)
