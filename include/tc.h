@@ -25,6 +25,7 @@
  */
 #ifndef TC_H
 #define TC_H
+#include <stddef.h>
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -103,6 +104,11 @@ tc_status tc_prior_eval(const float *volume, int n_slices, int n, const tc_prior
 /* One-shot form with exactly the problem statement's shape = create plan, tc_radon, destroy. */
 tc_status tc_radon1(const float *volume, int n_slices, int n, const float *angles, int n_angles, int n_det,
                     float center, float *sinogram);
+
+/* Page-locked host memory for callers without a CUDA runtime of their own (host-resident volumes of the streamed path):
+ * *ptr = `bytes` of pinned memory (not rounded up); release with tc_host_free.  TC_ENOMEM if it cannot be had. */
+tc_status tc_host_alloc(size_t bytes, void **ptr);
+tc_status tc_host_free(void *ptr);
 
 /* Kernel launches issued by this library on the calling thread since the last reset (for bench.py). */
 long long tc_launch_count(int reset);

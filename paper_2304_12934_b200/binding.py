@@ -54,9 +54,11 @@ lib.tc_launch_count.restype = ctypes.c_longlong
 lib.tc_last_sched_stats.argtypes = [_vp, ctypes.POINTER(tc_sched_stats)]
 lib.tc_profile.argtypes = [_vp, _ci]
 lib.tc_profile_read.argtypes = [_vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_longlong)]
+lib.tc_host_alloc.argtypes = [ctypes.c_size_t, ctypes.POINTER(_vp)]
+lib.tc_host_free.argtypes = [_vp]
 lib.tc_last_error.restype = ctypes.c_char_p
 for _f in ("tc_plan_create", "tc_plan_destroy", "tc_radon", "tc_backproject", "tc_fbp", "tc_mbir", "tc_power_iteration",
-           "tc_prior_eval", "tc_radon1", "tc_last_sched_stats", "tc_profile", "tc_profile_read"):
+           "tc_prior_eval", "tc_radon1", "tc_last_sched_stats", "tc_profile", "tc_profile_read", "tc_host_alloc", "tc_host_free"):
     getattr(lib, _f).restype = _ci
 
 
@@ -182,6 +184,22 @@ def radon1(volume, angles, n_det, center):
     out = _like(volume, (S, ang.size, n_det))
     _check(lib.tc_radon1(_ptr(volume), S, n, ang.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), ang.size, n_det, float(center), _ptr(out)))
     return out
+
+
+class PinnedArray:
+    """float32 numpy array on tc_host_alloc memory (exact size, page-locked); call free() when done with every view of it."""
+
+    def __init__(self, shape):
+        n = int(np.prod(shape))
+        self._p = _vp()
+        _check(lib.tc_host_alloc(n * 4, ctypes.byref(self._p)))
+        self.array = np.frombuffer((ctypes.c_float * n).from_address(self._p.value), dtype=np.float32).reshape(shape)
+
+    def free(self):
+        if self._p:
+            self.array = None
+            lib.tc_host_free(self._p)
+            self._p = None
 
 
 def launch_count(reset=False):

@@ -376,6 +376,17 @@ extern "C" tc_status tc_profile_read(tc_plan *p, double *ms, long long *launches
     return TC_OK;
 }
 
+extern "C" tc_status tc_host_alloc(size_t bytes, void **ptr) {
+    if (!ptr || bytes == 0) return fail(TC_EINVAL, "bad argument");
+    *ptr = nullptr;
+    if (cudaMallocHost(ptr, bytes) != cudaSuccess) { cudaGetLastError(); *ptr = nullptr; return fail(TC_ENOMEM, "tc_host_alloc: pinned host memory"); }
+    return TC_OK;
+}
+extern "C" tc_status tc_host_free(void *ptr) {
+    if (ptr && cudaFreeHost(ptr) != cudaSuccess) { cudaGetLastError(); return fail(TC_EINVAL, "tc_host_free: not a tc_host_alloc pointer"); }
+    return TC_OK;
+}
+
 static tc_status check_launch() {
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(TC_ECUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
