@@ -90,6 +90,7 @@ def stage_bytes(n, nd, na, S):
         "adj_spread": ng * na * nd * cell + ng * G * G * cell,
         "adj_cols": ng * (G * G + n * G) * cell,
         "adj_rows": ng * n * G * cell + S * n * n * 4,
+        "fwd_radial": ng * na * nd * cell + S * na * nd * 4,       # F4 as its own launch (tile-binned gather): reads cpol, writes the sinogram
     }
 
 

@@ -122,10 +122,10 @@ typedef struct { double h2d_s, compute_s, d2h_s, wall_s, overlap; long long h2d_
 tc_status tc_last_sched_stats(tc_plan *plan, tc_sched_stats *out);
 
 /* Per-kernel timing with CUDA events recorded on the launching stream around every NUFFT stage launch
- * (stages: 0 fwd_rows, 1 fwd_cols, 2 fwd_gather, 3 adj_radial, 4 adj_spread, 5 adj_cols, 6 adj_rows).
+ * (stages: 0 fwd_rows, 1 fwd_cols, 2 fwd_gather, 3 adj_radial, 4 adj_spread, 5 adj_cols, 6 adj_rows, 7 fwd_radial).
  * tc_profile switches recording on/off; tc_profile_read waits for the recorded events, returns summed
  * milliseconds and launch counts per stage (arrays of TC_N_STAGES, HOST) and clears the records. */
-#define TC_N_STAGES 7
+#define TC_N_STAGES 8
 tc_status tc_profile(tc_plan *plan, int enable);
 tc_status tc_profile_read(tc_plan *plan, double *ms, long long *launches);
 

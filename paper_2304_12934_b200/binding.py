@@ -7,7 +7,7 @@ import ctypes, os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libtc.so")
+_LIB_PATH = os.environ.get("TC_LIBTC", os.path.join(_HERE, "libtc.so"))
 if not os.path.exists(_LIB_PATH):
     raise ImportError("libtc.so not built: run `python -m paper_2304_12934_b200.build` (no CPU fallback exists)")
 lib = ctypes.CDLL(_LIB_PATH)
@@ -154,13 +154,13 @@ class Plan:
         _check(lib.tc_power_iteration(self._h, int(iters), ctypes.byref(v)))
         return v.value
 
-    STAGES = ("fwd_rows", "fwd_cols", "fwd_gather", "adj_radial", "adj_spread", "adj_cols", "adj_rows")
+    STAGES = ("fwd_rows", "fwd_cols", "fwd_gather", "adj_radial", "adj_spread", "adj_cols", "adj_rows", "fwd_radial")
 
     def profile(self, enable=True):
         _check(lib.tc_profile(self._h, 1 if enable else 0))
 
     def profile_read(self):
-        ms = (ctypes.c_double * 7)(); cnt = (ctypes.c_longlong * 7)()
+        ms = (ctypes.c_double * 8)(); cnt = (ctypes.c_longlong * 8)()
         _check(lib.tc_profile_read(self._h, ms, cnt))
         return {k: (ms[i], cnt[i]) for i, k in enumerate(self.STAGES)}
 

@@ -4,10 +4,10 @@ from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "libtc.so")
+LIB = os.environ.get("TC_LIBTC", os.path.join(HERE, "libtc.so"))      # TC_LIBTC: build / load another file (kernel variants)
 SOURCES = ["tc_api.cu", "kernels_nufft.cu", "kernels_mbir.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC", "-rdc=false"]
+FLAGS = os.environ.get("TC_NVCC_FLAGS", "").split() + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC", "-rdc=false"]
 
 
 def _stale():
@@ -21,7 +21,7 @@ def _stale():
 def build(force=False, verbose=False):
     if not force and not _stale():
         return LIB
-    bdir = os.path.join(HERE, "build")
+    bdir = os.path.join(HERE, "build", os.path.basename(LIB).replace(".so", ""))
     os.makedirs(bdir, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
 

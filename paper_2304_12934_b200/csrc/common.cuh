@@ -34,7 +34,31 @@ struct DevPlan {
     cudaStream_t side;            // the heavy-cell kernel runs beside the main spread kernel (disjoint cells): fork / join events
     cudaEvent_t ev_fork, ev_join;
     int J;                        // radial modes to try on each side of the nearest one: floor(3 sqrt2 / sc + 1/2)
+    // tile-binned forward gather (k_fwd_gather_tiles): polar samples sorted by the fine-grid tile that holds their first tap
+    int gt_ntx, gt_nty;           // tiles along the fast / slow axis
+    int gt_nlive;                 // tiles that hold at least one sample
+    const int *gt_tiles;          // [gt_nlive] tile ids (ty * gt_ntx + tx), most samples first
+    const unsigned *gt_start;     // [gt_ntx gt_nty + 1] offsets into gt_samples
+    const int4 *gt_samples;       // {a * nd + (m mod nd), (local base row << 16) | local base column, float bits of rx, of ry}
 };
+
+// Tile geometry of the binned gather: a tile owns the samples whose first tap (bx, by) falls into a GT_BX x GT_BY block of
+// fine-grid cells (x = the grid's fast, parity-split axis) and stages GT_CX x GT_CY cells (block + the W - 1 = 5 cells the
+// taps reach beyond it, rounded up to even) in shared memory, GT_NBUF tiles deep.
+#ifndef GT_BX
+#define GT_BX 42
+#endif
+#ifndef GT_BY
+#define GT_BY 42
+#endif
+#ifndef GT_NBUF
+#define GT_NBUF 2
+#endif
+constexpr int GT_CX = (GT_BX + 5 + 1) / 2 * 2, GT_CY = GT_BY + 5;
+static_assert(GT_BX % 2 == 0, "tile origins must keep the parity of the fast axis");
+__host__ __device__ inline int gt_min(int G) { return -G / 2 - 4; }            // centred coordinate of tile 0's first cell (even)
+__host__ __device__ inline int gt_ntx(int G) { return (G + 8 + GT_BX - 1) / GT_BX; }
+__host__ __device__ inline int gt_nty(int G) { return (G + 8 + GT_BY - 1) / GT_BY; }
 
 // Window polynomial coefficients (monomial in z, c[0] + c[1] z + ...), set by the plan.
 void set_kb_coeffs(const float *h);
@@ -46,6 +70,11 @@ void launch_fwd_rows(const DevPlan &d, const float *vol, int S, int ng, float2 *
 void launch_fwd_cols(const DevPlan &d, const float2 *rowbuf, int ng, float2 *grid, cudaStream_t st);
 // grid -> sino [S][na][nd]                       (F3 polar gather + F4 centre phase and inverse radial FFT)
 void launch_fwd_gather(const DevPlan &d, const float2 *grid, int S, int ng, float *sino, cudaStream_t st);
+// tile-binned form of F3 (+ F4 as its own launch): grid -> cpol [ng][na][nd][P] c64 -> sino
+void launch_gt_keys(const DevPlan &d, unsigned long long *keys, cudaStream_t st);
+void launch_gt_fill(const DevPlan &d, const unsigned long long *keys, unsigned nvalid, int4 *samples, unsigned *counts, cudaStream_t st);
+void launch_fwd_gather_tiles(const DevPlan &d, const float2 *grid, int ng, float2 *cpol, cudaStream_t st);
+void launch_fwd_radial(const DevPlan &d, const float2 *cpol, int S, int ng, float *sino, cudaStream_t st);
 // sino -> cpol [ng][na][nd][P] c64               (B1 radial FFT + conjugate phase)
 void launch_adj_radial(const DevPlan &d, const float *sino, int S, int ng, float2 *cpol, cudaStream_t st);
 // cpol -> grid                                   (B2 spread, evaluated per fine-grid cell: plain stores, no atomics)

@@ -1,0 +1,207 @@
+// Included by kernels_nufft.cu inside namespace tc: the forward polar gather (F3, eq. (7) reversed) binned by
+// fine-grid tile, and F4 (centre phase + inverse radial FFT, eq. (6) reversed P:L81) as its own launch.
+//
+// Why: evaluated ray by ray (k_fwd_gather) every one of a sample's 36 taps is its own scattered 32-byte request; the L1 data pipe
+// serves one 128-byte line per cycle whatever the request size, so that form is bound at 36 L1 wavefronts per sample and group,
+// with most of them going on to L2.  Here a CTA owns a GT_CX x GT_CY tile of fine-grid cells (72 KB), brings it into shared
+// memory ONCE with bulk asynchronous copies (cp.async.bulk -> UBLKCP, completion on an mbarrier; the rows are contiguous runs of
+// 32-byte cells because the fast axis is parity-split), and serves every polar sample whose 6 x 6 taps lie in the tile from
+// there: 128 bytes per shared-memory wavefront instead of 32, each cell crosses L2 -> SM once (plus the halo) instead of ~20
+// times.  Tiles are double-buffered: the copies of the next (tile, group) item run while the current one is being read.
+// The geometry (which samples a tile owns, their local tap base and fractional offsets) is plan-time data, shared by all groups
+// and calls.  The price is one HBM round trip of the polar coefficients (cpol: 2 x 32 B per sample and group, ~4 % of the
+// fine grid's bytes at config 4) between this kernel and k_fwd_radial.
+
+// ---- plan-time tables -------------------------------------------------------------------------------------------------------
+struct GtGeom { int bx, by; float rx, ry; };
+// first tap and offsets of sample (a, m), decided in float64 exactly as k_fwd_gather / the oracle decide them (readings G6, G19)
+__device__ __forceinline__ GtGeom gt_geom(const DevPlan &d, int a, int m) {
+    const double2 cs = d.cs[a];
+    const double kx = m * cs.x, ky = m * cs.y;
+    const double bxd = ceil(kx - 3.0), byd = ceil(ky - 3.0);
+    GtGeom g; g.bx = (int)bxd; g.by = (int)byd; g.rx = (float)(kx - bxd); g.ry = (float)(ky - byd);
+    return g;
+}
+
+// key = (tile << 32) | (a * nd + (m mod nd)); the excluded Nyquist mode (reading G2) sorts last
+__global__ void k_gt_keys(DevPlan d, unsigned long long *__restrict__ keys) {
+    const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    if (i >= (size_t)d.na * d.nd) return;
+    const int a = (int)(i / d.nd), mi = (int)(i - (size_t)a * d.nd), m = mi - d.nd / 2;
+    if (m == -d.nd / 2) { keys[i] = ~0ull; return; }
+    const GtGeom g = gt_geom(d, a, m);
+    const int tx = (g.bx - gt_min(d.G)) / GT_BX, ty = (g.by - gt_min(d.G)) / GT_BY;
+    keys[i] = ((unsigned long long)(ty * d.gt_ntx + tx) << 32) | (unsigned)(a * d.nd + (m < 0 ? m + d.nd : m));
+}
+
+__global__ void k_gt_fill(DevPlan d, const unsigned long long *__restrict__ keys, unsigned nvalid, int4 *__restrict__ samples,
+                          unsigned *__restrict__ counts) {
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nvalid) return;
+    const unsigned long long key = keys[i];
+    const int tile = (int)(key >> 32), idx = (int)(key & 0xffffffffu);
+    const int a = idx / d.nd, k = idx - a * d.nd, m = k < d.nd / 2 ? k : k - d.nd;
+    const GtGeom g = gt_geom(d, a, m);
+    const int tx = tile % d.gt_ntx, ty = tile / d.gt_ntx;
+    const int lx = g.bx - (gt_min(d.G) + tx * GT_BX), ly = g.by - (gt_min(d.G) + ty * GT_BY);   // in [0, GT_BX) x [0, GT_BY)
+    samples[i] = make_int4(idx, (ly << 16) | lx, __float_as_int(g.rx), __float_as_int(g.ry));
+    atomicAdd(&counts[tile], 1u);
+}
+
+// ---- mbarrier / bulk-copy primitives (PTX; sm_90+) --------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// global -> shared, `bytes` a multiple of 16, both addresses 16-byte aligned; completes `bytes` on the mbarrier
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// ---- the gather ---------------------------------------------------------------------------------------------------------------
+// The kernel's x is the fine grid's FAST (contiguous, parity-split) axis and y its slow axis (rows), as in k_fwd_gather.
+// Shared tile: cell (yl, xl) at ((yl * 2 + (xl & 1)) * (GT_CX / 2) + (xl >> 1)) * 32 bytes: the global row layout, cut to the tile.
+constexpr int GT_THREADS = 512;
+constexpr int GT_RUNS = GT_CY * 2;                           // (row, parity) runs of GT_CX / 2 cells each
+constexpr int GT_RUN_BYTES = (GT_CX / 2) * 32;
+constexpr int GT_TILE_BYTES = GT_CX * GT_CY * 32;
+static_assert(GT_RUNS <= GT_THREADS, "one thread per run");
+static_assert(GT_NBUF * GT_TILE_BYTES + 64 <= 227 * 1024, "tiles must fit in shared memory");
+
+__device__ __forceinline__ void gt_issue_tile(const DevPlan &d, const float2 *__restrict__ grid, int tile, int g, char *buf,
+                                              unsigned long long *bar) {
+    // threads 0 .. GT_RUNS-1: one run each (two copies when the run wraps around the end of the parity block)
+    const int r = threadIdx.x;
+    if (r >= GT_RUNS) return;
+    const int G = d.G, nh = G >> 1;
+    const int tx = tile % d.gt_ntx, ty = tile / d.gt_ntx;
+    const int yl = r >> 1, par = r & 1;
+    int Y = gt_min(G) + ty * GT_BY + yl;                                    // centred row -> storage row (taps wrap modulo G, reading G7)
+    Y %= G; if (Y < 0) Y += G;
+    int X = gt_min(G) + tx * GT_BX + par;                                   // first cell of the run (centred; same parity as par)
+    X %= G; if (X < 0) X += G;
+    const int pos0 = X >> 1;
+    const int len1 = min(GT_CX / 2, nh - pos0), len2 = GT_CX / 2 - len1;
+    const char *row = reinterpret_cast<const char *>(grid) + (((size_t)g * G + Y) * G + (size_t)par * nh) * 32;
+    char *dst = buf + (size_t)r * GT_RUN_BYTES;
+    mbar_arrive_expect_tx(bar, GT_RUN_BYTES);
+    bulk_g2s(dst, row + (size_t)pos0 * 32, len1 * 32, bar);
+    if (len2 > 0) bulk_g2s(dst + len1 * 32, row, len2 * 32, bar);
+}
+
+__global__ void __launch_bounds__(GT_THREADS, 1) k_fwd_gather_tiles(DevPlan d, const float2 *__restrict__ grid, int ng, float2 *__restrict__ cpol) {
+    extern __shared__ __align__(128) char gt_smem[];
+    char *tiles = gt_smem;                                                 // GT_NBUF x GT_TILE_BYTES
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(gt_smem + GT_NBUF * GT_TILE_BYTES);
+    if (threadIdx.x == 0)
+        for (int b = 0; b < GT_NBUF; ++b) mbar_init(&bars[b], GT_RUNS);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncthreads();
+    const int nitems = d.gt_nlive * ng;                                    // item w = (tile rank w / ng, group w % ng): heavy tiles first
+    const int pair = threadIdx.x >> 1, hp = threadIdx.x & 1;
+    const size_t gstride = (size_t)d.na * d.nd * 2;                        // float4 units per group of cpol
+    // prologue: the first GT_NBUF - 1 items of this CTA are on their way before the first one is read
+#pragma unroll
+    for (int j = 0; j < GT_NBUF - 1; ++j) {
+        const int wj = blockIdx.x + j * gridDim.x;
+        if (wj < nitems) gt_issue_tile(d, grid, d.gt_tiles[wj / ng], wj % ng, tiles + j * GT_TILE_BYTES, &bars[j]);
+    }
+    int k = 0;
+    for (int w = blockIdx.x; w < nitems; w += gridDim.x, ++k) {
+        const int wn = w + (GT_NBUF - 1) * gridDim.x, bn = (k + GT_NBUF - 1) % GT_NBUF;
+        if (wn < nitems) {                                                 // that buffer was released by the barrier that ended item k - 1
+            fence_proxy_async();
+            gt_issue_tile(d, grid, d.gt_tiles[wn / ng], wn % ng, tiles + bn * GT_TILE_BYTES, &bars[bn]);
+        }
+        const int tile = d.gt_tiles[w / ng], g = w % ng, bc = k % GT_NBUF;
+        const unsigned s0 = d.gt_start[tile], s1 = d.gt_start[tile + 1];
+        const float4 *tb = reinterpret_cast<const float4 *>(tiles + bc * GT_TILE_BYTES) + hp;
+        float4 *out = reinterpret_cast<float4 *>(cpol) + (size_t)g * gstride + hp;
+        int4 e = s0 + pair < s1 ? __ldg(&d.gt_samples[s0 + pair]) : make_int4(0, 0, 0, 0);
+        mbar_wait(&bars[bc], (k / GT_NBUF) & 1);
+#pragma unroll 1
+        for (unsigned s = s0 + pair; s < s1; s += GT_THREADS / 2) {
+            const int4 cur = e;
+            if (s + GT_THREADS / 2 < s1) e = __ldg(&d.gt_samples[s + GT_THREADS / 2]);
+            const int lx = cur.y & 0xffff, ly = cur.y >> 16;
+            const float rx = __int_as_float(cur.z), ry = __int_as_float(cur.w);
+            float wx[KB_W], wy[KB_W];
+#pragma unroll
+            for (int t = 0; t < KB_W; ++t) { wx[t] = kb_eval(rx - (float)t); wy[t] = kb_eval(ry - (float)t); }
+            int xo[KB_W];
+#pragma unroll
+            for (int t = 0; t < KB_W; ++t) { const int xl = lx + t; xo[t] = ((xl & 1) * (GT_CX / 2) + (xl >> 1)) * 2; }
+            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int ty = 0; ty < KB_W; ++ty) {
+                const float4 *row = tb + (size_t)(ly + ty) * GT_CX * 2;
+#pragma unroll
+                for (int tx = 0; tx < KB_W; ++tx) {
+                    const float4 v = row[xo[tx]];
+                    const float wgt2 = wy[ty] * wx[tx];
+                    acc.x = fmaf(wgt2, v.x, acc.x); acc.y = fmaf(wgt2, v.y, acc.y);
+                    acc.z = fmaf(wgt2, v.z, acc.z); acc.w = fmaf(wgt2, v.w, acc.w);
+                }
+            }
+            out[(size_t)cur.x * 2] = acc;
+        }
+        __syncthreads();                                                   // everybody is done reading this buffer
+    }
+}
+
+// F4: p[a][u] = (1/nd) sum_m c[a][m] e^{2 pi i m (u - centre)/nd}  (phase table ph_fwd carries 1/nd and the centre shift; its Nyquist
+// entry is 0 and that cell of cpol is never written, so it is not read either).  grid = (na, ng).
+template <class Cfg>
+__global__ void TC_LB k_fwd_radial(DevPlan d, const float2 *__restrict__ cpol, int S, float *__restrict__ sino) {
+    float2 *sm = reinterpret_cast<float2 *>(smem_f4);
+    const Cfg cfg = make_cfg<Cfg>(d.fD, 1);
+    const int a = blockIdx.x, g = blockIdx.y, nd = cfg.n(), pl = threadIdx.x & 3;
+    const int sre = 8 * g + 2 * pl;
+    const bool hre = sre < S, him = sre + 1 < S;
+    const float2 *in = cpol + ((size_t)g * d.na + a) * nd * 4 + pl;
+    float *ore = sino + ((size_t)sre * d.na + a) * nd, *oim = ore + (size_t)d.na * nd;
+    fft_line<true>(sm, cfg, d.twD,
+        [&](int k, bool) { return 2 * k == nd ? make_float2(0.f, 0.f) : cmul(__ldg(&in[(size_t)k * 4]), __ldg(&d.ph_fwd[k])); },
+        NoPre(), [&](int u, bool, float2 v, float2) {
+            if (hre) ore[u] = v.x;
+            if (him) oim[u] = v.y;
+        });
+}
+
+void launch_fwd_radial(const DevPlan &d, const float2 *cpol, int S, int ng, float *sino, cudaStream_t st) {
+    TC_LINE_LAUNCH(k_fwd_radial, 4, 1, 0, d.fD, dim3(d.na, ng), d, cpol, S, sino);
+}
+void launch_gt_keys(const DevPlan &d, unsigned long long *keys, cudaStream_t st) {
+    const size_t n = (size_t)d.na * d.nd;
+    k_gt_keys<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d, keys);
+}
+void launch_gt_fill(const DevPlan &d, const unsigned long long *keys, unsigned nvalid, int4 *samples, unsigned *counts, cudaStream_t st) {
+    k_gt_fill<<<(nvalid + 255) / 256, 256, 0, st>>>(d, keys, nvalid, samples, counts);
+}
+void launch_fwd_gather_tiles(const DevPlan &d, const float2 *grid, int ng, float2 *cpol, cudaStream_t st) {
+    static int n_sm = 0;
+    if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
+    const size_t sh = GT_NBUF * GT_TILE_BYTES + 64;
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(k_fwd_gather_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh); attr = true; }
+    const int nitems = d.gt_nlive * ng;
+    if (nitems <= 0) return;
+    k_fwd_gather_tiles<<<std::min(n_sm, nitems), GT_THREADS, sh, st>>>(d, grid, ng, cpol);
+    TC_COUNT_LAUNCH();
+}

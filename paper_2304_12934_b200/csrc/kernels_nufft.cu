@@ -6,6 +6,7 @@
 // transform (the Nyquist radial mode is excluded, reading G2, so nothing leaks between them).
 // Every kernel below reads and writes whole 32-byte cells (or 16-byte halves of them).
 #include <cstdlib>
+#include <algorithm>
 #include "common.cuh"
 #include "fft_line.cuh"
 
@@ -166,5 +167,6 @@ __global__ void TC_LB2 k_adj_rows(DevPlan d, const float2 *__restrict__ rowbuf, 
 }
 
 #include "kernels_polar.cuh"
+#include "kernels_gather_tiles.cuh"
 
 }  // namespace tc

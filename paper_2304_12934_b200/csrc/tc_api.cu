@@ -10,6 +10,7 @@
 #include "../../include/tc.h"
 #include "common.cuh"
 #include <cub/device/device_scan.cuh>
+#include <cub/device/device_radix_sort.cuh>
 
 using namespace tc;
 
@@ -44,6 +45,8 @@ struct tc_plan {
     int2 *taps = nullptr;
     unsigned *heavy = nullptr;
     long long n_taps = 0;
+    int *gt_tiles = nullptr; unsigned *gt_start = nullptr; int4 *gt_samples = nullptr;   // tile-binned gather tables
+    bool gather_tiles = true;     // F3 as k_fwd_gather_tiles + k_fwd_radial (default) or as the fused ray-by-ray k_fwd_gather (TC_GATHER=ray)
     // scratch
     int ng_alloc = 0;
     float2 *rowbuf = nullptr, *grid = nullptr, *cpol = nullptr;
@@ -278,6 +281,44 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
         e = cudaDeviceSynchronize();
         if (e != cudaSuccess) { tc_plan_destroy(p); return fail(TC_ECUDA, std::string("spread tap lists: ") + cudaGetErrorString(e)); }
     }
+    {   // tile-binned gather: samples sorted by tile (radix sort of (tile, sample) keys), tile offsets, tiles ordered by load
+        const size_t ns = (size_t)na * nd;
+        d.gt_ntx = gt_ntx(G); d.gt_nty = gt_nty(G);
+        const int ntile = d.gt_ntx * d.gt_nty;
+        unsigned long long *keys = nullptr, *keys2 = nullptr; void *tmp = nullptr; size_t tmp_bytes = 0; unsigned *counts = nullptr;
+        const int end_bit = 32 + std::max(1, (int)std::ceil(std::log2((double)ntile + 1)));
+        const unsigned nvalid = (unsigned)((size_t)na * (nd - 1));           // all but the Nyquist mode of every angle
+        e = cudaMalloc((void **)&keys, ns * sizeof(unsigned long long));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&keys2, ns * sizeof(unsigned long long));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&counts, (size_t)ntile * sizeof(unsigned));
+        if (e == cudaSuccess) e = cudaMemset(counts, 0, (size_t)ntile * sizeof(unsigned));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&p->gt_samples, (size_t)std::max(nvalid, 1u) * sizeof(int4));
+        if (e == cudaSuccess) {
+            launch_gt_keys(d, keys, nullptr);
+            cub::DeviceRadixSort::SortKeys(nullptr, tmp_bytes, keys, keys2, (int)ns, 0, 64);
+            e = cudaMalloc(&tmp, tmp_bytes);
+        }
+        if (e == cudaSuccess) e = cub::DeviceRadixSort::SortKeys(tmp, tmp_bytes, keys, keys2, (int)ns, 0, 64);
+        (void)end_bit;
+        if (e == cudaSuccess) { launch_gt_fill(d, keys2, nvalid, p->gt_samples, counts, nullptr); e = cudaDeviceSynchronize(); }
+        std::vector<unsigned> hc(ntile), hs(ntile + 1, 0);
+        if (e == cudaSuccess) e = cudaMemcpy(hc.data(), counts, (size_t)ntile * sizeof(unsigned), cudaMemcpyDeviceToHost);
+        cudaFree(keys); cudaFree(keys2); cudaFree(tmp); cudaFree(counts);
+        std::vector<int> live;
+        if (e == cudaSuccess) {
+            for (int t = 0; t < ntile; ++t) { hs[t + 1] = hs[t] + hc[t]; if (hc[t]) live.push_back(t); }
+            std::stable_sort(live.begin(), live.end(), [&](int x, int y) { return hc[x] > hc[y]; });
+            if (hs[ntile] != nvalid) { tc_plan_destroy(p); return fail(TC_ECUDA, "gather tiles: sample count mismatch"); }
+            if (live.empty()) live.push_back(0);
+            e = upload(&p->gt_tiles, live);
+            if (e == cudaSuccess) e = upload(&p->gt_start, hs);
+        }
+        if (e != cudaSuccess) { tc_plan_destroy(p); return fail(e == cudaErrorMemoryAllocation ? TC_ENOMEM : TC_ECUDA, std::string("gather tiles: ") + cudaGetErrorString(e)); }
+        d.gt_nlive = nvalid ? (int)live.size() : 0;
+        d.gt_tiles = p->gt_tiles; d.gt_start = p->gt_start; d.gt_samples = p->gt_samples;
+        const char *env = std::getenv("TC_GATHER");
+        p->gather_tiles = !(env && std::string(env) == "ray");
+    }
     *out = p;
     return TC_OK;
 }
@@ -294,6 +335,7 @@ extern "C" tc_status tc_plan_destroy(tc_plan *p) {
     free_scratch(p);
     cudaFree(p->twG); cudaFree(p->twD); cudaFree(p->ph_fwd); cudaFree(p->ph_adj); cudaFree(p->ph_fbp[0]); cudaFree(p->ph_fbp[1]); cudaFree(p->deapod);
     cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc); cudaFree(p->tile_rng); cudaFree(p->tile_nr); cudaFree(p->tap_offs); cudaFree(p->taps); cudaFree(p->heavy);
+    cudaFree(p->gt_tiles); cudaFree(p->gt_start); cudaFree(p->gt_samples);
     if (p->d.side) cudaStreamDestroy(p->d.side);
     if (p->d.ev_fork) cudaEventDestroy(p->d.ev_fork);
     if (p->d.ev_join) cudaEventDestroy(p->d.ev_join);
@@ -344,7 +386,12 @@ static void forward_slab(tc_plan *p, const float *vol, int S, float *sino, cudaS
     const int ng = (S + 7) / 8;
     STAGE(0, launch_fwd_rows(p->d, vol, S, ng, p->rowbuf, st));
     STAGE(1, launch_fwd_cols(p->d, p->rowbuf, ng, p->grid, st));
-    STAGE(2, launch_fwd_gather(p->d, p->grid, S, ng, sino, st));
+    if (p->gather_tiles) {
+        STAGE(2, launch_fwd_gather_tiles(p->d, p->grid, ng, p->cpol, st));
+        STAGE(7, launch_fwd_radial(p->d, p->cpol, S, ng, sino, st));
+    } else {
+        STAGE(2, launch_fwd_gather(p->d, p->grid, S, ng, sino, st));
+    }
 }
 // B1-B4.  tc_fbp is the same pipeline with the FBP-weighted phase table in place of ph_adj (one multiply in B1): p->fbp_filter >= 0.
 static void adjoint_slab(tc_plan *p, const float *sino, int S, float *vol, cudaStream_t st) {
