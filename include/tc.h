@@ -85,6 +85,14 @@ tc_status tc_backproject(tc_plan *plan, const float *sinogram, int n_slices, flo
 #define TC_FILTER_HANN 1
 tc_status tc_fbp(tc_plan *plan, const float *sinogram, int n_slices, int filter, float *volume, void *cuda_stream);
 
+/* Pre-pass for measured data ("b = -log(I / I0)", P:L129 sinogram order): Beer-Lambert transform and the reorder from
+ * projection order, proj[n_angles][n_slices][n_det] as a detector delivers it, to sinogram[n_slices][n_angles][n_det]:
+ *   sinogram[s][a][u] = -log(max((proj[a][s][u] - dark[s][u]) / (flat[s][u] - dark[s][u]), floor)),
+ * flat (I0) and dark are [n_slices][n_det], nullable (1 and 0).  floor > 0 guards dead or saturated pixels.  All device or all
+ * host pointers; device calls are ordered on cuda_stream. */
+tc_status tc_preprocess(const float *proj, const float *flat, const float *dark, int n_angles, int n_slices, int n_det,
+                        float floor, float *sinogram, void *cuda_stream);
+
 /* `iters` iterations of the monotone accelerated gradient method with restart on
  * F(f) = 1/2 ||A f - b||^2 + lambda H(f) from f = 0.  volume: out.  log: HOST pointer, nullable,
  * `iters` records.  Synchronous (returns when `volume` is complete).

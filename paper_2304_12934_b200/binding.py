@@ -54,11 +54,12 @@ lib.tc_launch_count.restype = ctypes.c_longlong
 lib.tc_last_sched_stats.argtypes = [_vp, ctypes.POINTER(tc_sched_stats)]
 lib.tc_profile.argtypes = [_vp, _ci]
 lib.tc_profile_read.argtypes = [_vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_longlong)]
+lib.tc_preprocess.argtypes = [_vp, _vp, _vp, _ci, _ci, _ci, ctypes.c_float, _vp, _vp]
 lib.tc_host_alloc.argtypes = [ctypes.c_size_t, ctypes.POINTER(_vp)]
 lib.tc_host_free.argtypes = [_vp]
 lib.tc_last_error.restype = ctypes.c_char_p
 for _f in ("tc_plan_create", "tc_plan_destroy", "tc_radon", "tc_backproject", "tc_fbp", "tc_mbir", "tc_power_iteration",
-           "tc_prior_eval", "tc_radon1", "tc_last_sched_stats", "tc_profile", "tc_profile_read", "tc_host_alloc", "tc_host_free"):
+           "tc_prior_eval", "tc_radon1", "tc_last_sched_stats", "tc_profile", "tc_profile_read", "tc_host_alloc", "tc_host_free", "tc_preprocess"):
     getattr(lib, _f).restype = _ci
 
 
@@ -176,6 +177,15 @@ def prior_eval(volume, prior, want_grad=True):
     val = ctypes.c_double()
     _check(lib.tc_prior_eval(_ptr(volume), S, n, ctypes.byref(prior), _ptr(grad) if want_grad else None, ctypes.byref(val)))
     return val.value, grad
+
+
+def preprocess(proj, flat=None, dark=None, floor=1e-6):
+    """tc_preprocess: proj (Na, S, Nd) intensities -> sinogram (S, Na, Nd) line integrals."""
+    na, S, nd = proj.shape
+    out = _like(proj, (S, na, nd))
+    _check(lib.tc_preprocess(_ptr(proj), None if flat is None else _ptr(flat), None if dark is None else _ptr(dark), na, S, nd,
+                             float(floor), _ptr(out), _stream(proj)))
+    return out
 
 
 def radon1(volume, angles, n_det, center):

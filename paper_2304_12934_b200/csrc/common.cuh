@@ -37,6 +37,7 @@ struct DevPlan {
     // tile-binned forward gather (k_fwd_gather_tiles): polar samples sorted by the fine-grid tile that holds their first tap
     int gt_ntx, gt_nty;           // tiles along the fast / slow axis
     int gt_nlive;                 // tiles that hold at least one sample
+    int gt_nh, gt_nm;             // ranks [0, gt_nh): one group per work item, [gt_nh, gt_nm): four, the rest: sixteen
     const int *gt_tiles;          // [gt_nlive] tile ids (ty * gt_ntx + tx), most samples first
     const unsigned *gt_start;     // [gt_ntx gt_nty + 1] offsets into gt_samples
     const int4 *gt_samples;       // {a * nd + (m mod nd), (local base row << 16) | local base column, float bits of rx, of ry}
@@ -46,10 +47,10 @@ struct DevPlan {
 // fine-grid cells (x = the grid's fast, parity-split axis) and stages GT_CX x GT_CY cells (block + the W - 1 = 5 cells the
 // taps reach beyond it, rounded up to even) in shared memory, GT_NBUF tiles deep.
 #ifndef GT_BX
-#define GT_BX 42
+#define GT_BX 90
 #endif
 #ifndef GT_BY
-#define GT_BY 42
+#define GT_BY 26
 #endif
 #ifndef GT_NBUF
 #define GT_NBUF 2
@@ -114,6 +115,8 @@ void launch_sumsq(const float *v, size_t n, double *acc, int slot, cudaStream_t 
 // acc[slot] += sum g (z - x)   (gradient restart test)
 void launch_dot_gzx(const float *g, const float *z, const float *x, size_t n, double *acc, int slot, cudaStream_t st);
 void launch_scale(float *v, float a, size_t n, cudaStream_t st);
+// sino[s][a][u] = -log(max((proj[a][s][u] - dark[s][u]) / (flat[s][u] - dark[s][u]), floor))   (Beer-Lambert + reorder)
+void launch_preprocess(const float *proj, const float *flat, const float *dark, int na, int S, int nd, float floor_, float *sino, cudaStream_t st);
 
 long long &launch_counter();
 

@@ -7,7 +7,7 @@
 // memory ONCE with bulk asynchronous copies (cp.async.bulk -> UBLKCP, completion on an mbarrier; the rows are contiguous runs of
 // 32-byte cells because the fast axis is parity-split), and serves every polar sample whose 6 x 6 taps lie in the tile from
 // there: 128 bytes per shared-memory wavefront instead of 32, each cell crosses L2 -> SM once (plus the halo) instead of ~20
-// times.  Tiles are double-buffered: the copies of the next (tile, group) item run while the current one is being read.
+// times.  Tiles are multi-buffered: the copies of the next (tile, group) loads run while the current one is being read.
 // The geometry (which samples a tile owns, their local tap base and fractional offsets) is plan-time data, shared by all groups
 // and calls.  The price is one HBM round trip of the polar coefficients (cpol: 2 x 32 B per sample and group, ~4 % of the
 // fine grid's bytes at config 4) between this kernel and k_fwd_radial.
@@ -77,7 +77,7 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // ---- the gather ---------------------------------------------------------------------------------------------------------------
 // The kernel's x is the fine grid's FAST (contiguous, parity-split) axis and y its slow axis (rows), as in k_fwd_gather.
 // Shared tile: cell (yl, xl) at ((yl * 2 + (xl & 1)) * (GT_CX / 2) + (xl >> 1)) * 32 bytes: the global row layout, cut to the tile.
-constexpr int GT_THREADS = 512;
+constexpr int GT_THREADS = 1024;
 constexpr int GT_RUNS = GT_CY * 2;                           // (row, parity) runs of GT_CX / 2 cells each
 constexpr int GT_RUN_BYTES = (GT_CX / 2) * 32;
 constexpr int GT_TILE_BYTES = GT_CX * GT_CY * 32;
@@ -105,6 +105,66 @@ __device__ __forceinline__ void gt_issue_tile(const DevPlan &d, const float2 *__
     if (len2 > 0) bulk_g2s(dst + len1 * 32, row, len2 * 32, bar);
 }
 
+// Work items.  Tiles are sorted by sample count (most first).  One item = one tile for a run of GC consecutive groups, so that
+// the thread pair that owns a sample evaluates its window weights ONCE and reuses them for every group of the run (the geometry
+// is the same for all groups); the tiles near the origin, where every ray passes, are cut into shorter runs so that no item is
+// more than a few per cent of a CTA's share: tile ranks [0, nh): GC = 1, [nh, nm): GC = 4, the rest: GC = 16.
+// Items are dealt to the CTAs round robin, heavy ones first; a CTA streams the (tile, group) loads of its items through
+// GT_NBUF shared-memory buffers, GT_NBUF - 1 loads ahead of the one being read.
+struct GtCursor {
+    int w, j, tile, g0, gc;            // item, position in its run of groups, tile id, first group, groups in this item
+    bool valid;
+};
+__device__ __forceinline__ void gt_decode(const DevPlan &d, int ng, GtCursor &c) {
+    const int c4 = (ng + 3) >> 2, c16 = (ng + 15) >> 4;
+    const int nA = d.gt_nh * ng, nB = (d.gt_nm - d.gt_nh) * c4, nC = (d.gt_nlive - d.gt_nm) * c16;
+    c.j = 0;
+    c.valid = c.w < nA + nB + nC;
+    if (!c.valid) return;
+    int rank, step;
+    if (c.w < nA) { rank = c.w / ng; c.g0 = c.w - rank * ng; step = 1; }
+    else if (c.w < nA + nB) { const int v = c.w - nA; rank = v / c4; c.g0 = (v - rank * c4) * 4; rank += d.gt_nh; step = 4; }
+    else { const int v = c.w - nA - nB; rank = v / c16; c.g0 = (v - rank * c16) * 16; rank += d.gt_nm; step = 16; }
+    c.gc = min(step, ng - c.g0);
+    c.tile = d.gt_tiles[rank];
+}
+__device__ __forceinline__ void gt_advance(const DevPlan &d, int ng, GtCursor &c) {
+    if (++c.j < c.gc) return;
+    c.w += gridDim.x;
+    gt_decode(d, ng, c);
+}
+
+struct GtTaps { float wx[KB_W], wy[KB_W]; int base; };          // window weights and the float4 index of tap (0, 0) in the tile
+__device__ __forceinline__ GtTaps gt_taps(const int4 e) {
+    GtTaps t;
+    const int lx = e.y & 0xffff, ly = e.y >> 16;
+    const float rx = __int_as_float(e.z), ry = __int_as_float(e.w);
+#pragma unroll
+    for (int k = 0; k < KB_W; ++k) { t.wx[k] = kb_eval(rx - (float)k); t.wy[k] = kb_eval(ry - (float)k); }
+    // cell (yl, xl) sits at float4 index (yl * GT_CX + (xl & 1) * (GT_CX / 2) + (xl >> 1)) * 2: taps t and t + 2 along x are neighbours
+    t.base = (ly * GT_CX + (lx & 1) * (GT_CX / 2) + (lx >> 1)) * 2;
+    return t;
+}
+// sum over the 6 x 6 taps; `odd` = parity of the first tap's column (decides on which side of the parity split taps 1, 3, 5 lie)
+__device__ __forceinline__ float4 gt_apply(const float4 *__restrict__ tb, const GtTaps &t, bool odd) {
+    // x taps 0, 2, 4 share the parity of lx and sit at +0, +1, +2 cells; taps 1, 3, 5 have the other parity: the other run, and one cell
+    // further along when lx is odd
+    const int o1 = odd ? (1 - GT_CX / 2) * 2 : (GT_CX / 2) * 2;
+    const float4 *p0 = tb + t.base, *p1 = p0 + o1;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int ty = 0; ty < KB_W; ++ty) {
+#pragma unroll
+        for (int tx = 0; tx < KB_W; ++tx) {
+            const float4 v = (tx & 1) ? p1[ty * GT_CX * 2 + (tx >> 1) * 2] : p0[ty * GT_CX * 2 + (tx >> 1) * 2];
+            const float w2 = t.wy[ty] * t.wx[tx];
+            acc.x = fmaf(w2, v.x, acc.x); acc.y = fmaf(w2, v.y, acc.y);
+            acc.z = fmaf(w2, v.z, acc.z); acc.w = fmaf(w2, v.w, acc.w);
+        }
+    }
+    return acc;
+}
+
 __global__ void __launch_bounds__(GT_THREADS, 1) k_fwd_gather_tiles(DevPlan d, const float2 *__restrict__ grid, int ng, float2 *__restrict__ cpol) {
     extern __shared__ __align__(128) char gt_smem[];
     char *tiles = gt_smem;                                                 // GT_NBUF x GT_TILE_BYTES
@@ -113,55 +173,46 @@ __global__ void __launch_bounds__(GT_THREADS, 1) k_fwd_gather_tiles(DevPlan d, c
         for (int b = 0; b < GT_NBUF; ++b) mbar_init(&bars[b], GT_RUNS);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
-    const int nitems = d.gt_nlive * ng;                                    // item w = (tile rank w / ng, group w % ng): heavy tiles first
     const int pair = threadIdx.x >> 1, hp = threadIdx.x & 1;
     const size_t gstride = (size_t)d.na * d.nd * 2;                        // float4 units per group of cpol
-    // prologue: the first GT_NBUF - 1 items of this CTA are on their way before the first one is read
+    GtCursor cons, prod;
+    cons.w = blockIdx.x; gt_decode(d, ng, cons);
+    prod = cons;
+    // prologue: GT_NBUF - 1 loads are on their way before the first one is read
 #pragma unroll
-    for (int j = 0; j < GT_NBUF - 1; ++j) {
-        const int wj = blockIdx.x + j * gridDim.x;
-        if (wj < nitems) gt_issue_tile(d, grid, d.gt_tiles[wj / ng], wj % ng, tiles + j * GT_TILE_BYTES, &bars[j]);
-    }
-    int k = 0;
-    for (int w = blockIdx.x; w < nitems; w += gridDim.x, ++k) {
-        const int wn = w + (GT_NBUF - 1) * gridDim.x, bn = (k + GT_NBUF - 1) % GT_NBUF;
-        if (wn < nitems) {                                                 // that buffer was released by the barrier that ended item k - 1
+    for (int j = 0; j < GT_NBUF - 1; ++j)
+        if (prod.valid) { gt_issue_tile(d, grid, prod.tile, prod.g0 + prod.j, tiles + j * GT_TILE_BYTES, &bars[j]); gt_advance(d, ng, prod); }
+    GtTaps mine;                                                           // this pair's first sample of the current tile, kept across its groups
+    int mine_idx = -1; bool mine_odd = false;
+    unsigned s0 = 0, s1 = 0;
+    for (int k = 0; cons.valid; ++k) {
+        if (prod.valid) {                                                  // that buffer was released by the barrier that ended load k - 1
             fence_proxy_async();
-            gt_issue_tile(d, grid, d.gt_tiles[wn / ng], wn % ng, tiles + bn * GT_TILE_BYTES, &bars[bn]);
+            const int bn = (k + GT_NBUF - 1) % GT_NBUF;
+            gt_issue_tile(d, grid, prod.tile, prod.g0 + prod.j, tiles + bn * GT_TILE_BYTES, &bars[bn]);
+            gt_advance(d, ng, prod);
         }
-        const int tile = d.gt_tiles[w / ng], g = w % ng, bc = k % GT_NBUF;
-        const unsigned s0 = d.gt_start[tile], s1 = d.gt_start[tile + 1];
-        const float4 *tb = reinterpret_cast<const float4 *>(tiles + bc * GT_TILE_BYTES) + hp;
-        float4 *out = reinterpret_cast<float4 *>(cpol) + (size_t)g * gstride + hp;
-        int4 e = s0 + pair < s1 ? __ldg(&d.gt_samples[s0 + pair]) : make_int4(0, 0, 0, 0);
-        mbar_wait(&bars[bc], (k / GT_NBUF) & 1);
-#pragma unroll 1
-        for (unsigned s = s0 + pair; s < s1; s += GT_THREADS / 2) {
-            const int4 cur = e;
-            if (s + GT_THREADS / 2 < s1) e = __ldg(&d.gt_samples[s + GT_THREADS / 2]);
-            const int lx = cur.y & 0xffff, ly = cur.y >> 16;
-            const float rx = __int_as_float(cur.z), ry = __int_as_float(cur.w);
-            float wx[KB_W], wy[KB_W];
-#pragma unroll
-            for (int t = 0; t < KB_W; ++t) { wx[t] = kb_eval(rx - (float)t); wy[t] = kb_eval(ry - (float)t); }
-            int xo[KB_W];
-#pragma unroll
-            for (int t = 0; t < KB_W; ++t) { const int xl = lx + t; xo[t] = ((xl & 1) * (GT_CX / 2) + (xl >> 1)) * 2; }
-            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-            for (int ty = 0; ty < KB_W; ++ty) {
-                const float4 *row = tb + (size_t)(ly + ty) * GT_CX * 2;
-#pragma unroll
-                for (int tx = 0; tx < KB_W; ++tx) {
-                    const float4 v = row[xo[tx]];
-                    const float wgt2 = wy[ty] * wx[tx];
-                    acc.x = fmaf(wgt2, v.x, acc.x); acc.y = fmaf(wgt2, v.y, acc.y);
-                    acc.z = fmaf(wgt2, v.z, acc.z); acc.w = fmaf(wgt2, v.w, acc.w);
-                }
+        if (cons.j == 0) {                                                 // new tile: weights of this pair's first sample
+            s0 = d.gt_start[cons.tile]; s1 = d.gt_start[cons.tile + 1];
+            mine_idx = -1;
+            if (s0 + pair < s1) {
+                const int4 e = __ldg(&d.gt_samples[s0 + pair]);
+                mine = gt_taps(e); mine_idx = e.x; mine_odd = e.y & 1;
             }
-            out[(size_t)cur.x * 2] = acc;
+        }
+        const int bc = k % GT_NBUF;
+        const float4 *tb = reinterpret_cast<const float4 *>(tiles + bc * GT_TILE_BYTES) + hp;
+        float4 *out = reinterpret_cast<float4 *>(cpol) + (size_t)(cons.g0 + cons.j) * gstride + hp;
+        mbar_wait(&bars[bc], (k / GT_NBUF) & 1);
+        if (mine_idx >= 0) out[(size_t)mine_idx * 2] = gt_apply(tb, mine, mine_odd);
+#pragma unroll 1
+        for (unsigned s = s0 + pair + GT_THREADS / 2; s < s1; s += GT_THREADS / 2) {       // crowded tiles: the further samples of this pair
+            const int4 e = __ldg(&d.gt_samples[s]);
+            const GtTaps t = gt_taps(e);
+            out[(size_t)e.x * 2] = gt_apply(tb, t, e.y & 1);
         }
         __syncthreads();                                                   // everybody is done reading this buffer
+        gt_advance(d, ng, cons);
     }
 }
 
@@ -200,7 +251,7 @@ void launch_fwd_gather_tiles(const DevPlan &d, const float2 *grid, int ng, float
     const size_t sh = GT_NBUF * GT_TILE_BYTES + 64;
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(k_fwd_gather_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh); attr = true; }
-    const int nitems = d.gt_nlive * ng;
+    const int nitems = d.gt_nh * ng + (d.gt_nm - d.gt_nh) * ((ng + 3) / 4) + (d.gt_nlive - d.gt_nm) * ((ng + 15) / 16);
     if (nitems <= 0) return;
     k_fwd_gather_tiles<<<std::min(n_sm, nitems), GT_THREADS, sh, st>>>(d, grid, ng, cpol);
     TC_COUNT_LAUNCH();

@@ -93,6 +93,21 @@ __global__ void k_dot_gzx(const float *__restrict__ g, const float *__restrict__
         s += (double)g[i] * ((double)z[i] - (double)x[i]);
     block_reduce_to(s, partials);
 }
+// Beer-Lambert pre-pass + projection -> sinogram reorder: sino[s][a][u] = -log(max((I - dark) / (flat - dark), floor)),
+// I = proj[a][s][u]; flat / dark are [s][u] (nullable: 1 / 0).  One thread per (a, s, u): both sides are contiguous along u.
+__global__ void k_preprocess(const float *__restrict__ proj, const float *__restrict__ flat, const float *__restrict__ dark,
+                             int na, int S, int nd, float floor_, float *__restrict__ sino) {
+    const size_t n = (size_t)na * S * nd;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const int u = (int)(i % nd);
+        const size_t as = i / nd;
+        const int s = (int)(as % S), a = (int)(as / S);
+        const size_t su = (size_t)s * nd + u;
+        const float dk = dark ? dark[su] : 0.f, fl = flat ? flat[su] : 1.f;
+        const float t = fmaxf((proj[i] - dk) / (fl - dk), floor_);
+        sino[((size_t)s * na + a) * nd + u] = -logf(t);
+    }
+}
 __global__ void k_scale(float *v, float a, size_t n) {
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) v[i] *= a;
 }
@@ -400,6 +415,9 @@ void launch_sumsq(const float *v, size_t n, double *acc, int slot, cudaStream_t 
 void launch_dot_gzx(const float *g, const float *z, const float *x, size_t n, double *acc, int slot, cudaStream_t st) {
     k_dot_gzx<<<RED_BLOCKS, RED_THREADS, 0, st>>>(g, z, x, n, acc + 16); TC_COUNT_LAUNCH();
     final_reduce(acc, slot, 1.0, st);
+}
+void launch_preprocess(const float *proj, const float *flat, const float *dark, int na, int S, int nd, float floor_, float *sino, cudaStream_t st) {
+    k_preprocess<<<ew_blocks((size_t)na * S * nd), 256, 0, st>>>(proj, flat, dark, na, S, nd, floor_, sino); TC_COUNT_LAUNCH();
 }
 void launch_scale(float *v, float a, size_t n, cudaStream_t st) {
     k_scale<<<ew_blocks(n), 256, 0, st>>>(v, a, n); TC_COUNT_LAUNCH();

@@ -312,9 +312,59 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
             if (live.empty()) live.push_back(0);
             e = upload(&p->gt_tiles, live);
             if (e == cudaSuccess) e = upload(&p->gt_start, hs);
+            // Order the samples of every tile so that the four samples a quarter-warp reads together (one 128-byte shared-memory
+            // wavefront = four 32-byte cells) never share a bank group: a cell's bank group is (column >> 1) mod 4, the same for
+            // every tap once the first tap's column is fixed modulo 8, so a quartet takes its samples from the four residues of one
+            // parity (0, 2, 4, 6 or 1, 3, 5, 7).  Queues are filled in (angle, mode) order, so quartets stay close in cpol.
+            std::vector<int4> hsmp(std::max(nvalid, 1u));
+            if (e == cudaSuccess) e = cudaMemcpy(hsmp.data(), p->gt_samples, (size_t)nvalid * sizeof(int4), cudaMemcpyDeviceToHost);
+            if (e == cudaSuccess) {
+                std::vector<int4> bins[8], outv;
+                for (int t = 0; t < ntile; ++t) {
+                    if (!hc[t]) continue;
+                    for (auto &b : bins) b.clear();
+                    outv.clear();
+                    for (unsigned i = hs[t]; i < hs[t + 1]; ++i) bins[hsmp[i].y & 7].push_back(hsmp[i]);
+                    size_t head[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+                    for (int par = 0; par < 2; ++par)
+                        for (;;) {
+                            bool all = true;
+                            for (int q = 0; q < 4; ++q) all = all && head[par + 2 * q] < bins[par + 2 * q].size();
+                            if (!all) break;
+                            for (int q = 0; q < 4; ++q) { outv.push_back(bins[par + 2 * q][head[par + 2 * q]]); ++head[par + 2 * q]; }
+                        }
+                    for (;;) {                                     // leftovers: up to four samples from the fullest queues with distinct bank groups
+                        int pick[4] = {-1, -1, -1, -1}; bool any = false;
+                        for (int q = 0; q < 4; ++q) {
+                            size_t best = 0;
+                            for (int par = 0; par < 2; ++par) { const int b = par + 2 * q; const size_t left = bins[b].size() - head[b]; if (left > best) { best = left; pick[q] = b; } }
+                            any = any || pick[q] >= 0;
+                        }
+                        if (!any) break;
+                        int placed = 0;
+                        for (int q = 0; q < 4; ++q) if (pick[q] >= 0) { outv.push_back(bins[pick[q]][head[pick[q]]]); ++head[pick[q]]; ++placed; }
+                        for (; placed < 4; ++placed) {             // fill the quartet from whatever is left (conflicts, rare)
+                            int b = -1; size_t best = 0;
+                            for (int k2 = 0; k2 < 8; ++k2) { const size_t left = bins[k2].size() - head[k2]; if (left > best) { best = left; b = k2; } }
+                            if (b < 0) break;
+                            outv.push_back(bins[b][head[b]]); ++head[b];
+                        }
+                    }
+                    std::copy(outv.begin(), outv.end(), hsmp.begin() + hs[t]);
+                }
+                e = cudaMemcpy(p->gt_samples, hsmp.data(), (size_t)nvalid * sizeof(int4), cudaMemcpyHostToDevice);
+            }
         }
         if (e != cudaSuccess) { tc_plan_destroy(p); return fail(e == cudaErrorMemoryAllocation ? TC_ENOMEM : TC_ECUDA, std::string("gather tiles: ") + cudaGetErrorString(e)); }
         d.gt_nlive = nvalid ? (int)live.size() : 0;
+        {   // cut the crowded tiles into shorter group runs: a 16-group item should stay below ~5 % of one CTA's share of the samples
+            const unsigned lim16 = std::max(64u, nvalid / (148u * 20u));
+            d.gt_nh = d.gt_nm = 0;
+            for (int r = 0; r < d.gt_nlive; ++r) {
+                if (hc[live[r]] > 4 * lim16) d.gt_nh = r + 1;
+                if (hc[live[r]] > lim16) d.gt_nm = r + 1;
+            }
+        }
         d.gt_tiles = p->gt_tiles; d.gt_start = p->gt_start; d.gt_samples = p->gt_samples;
         const char *env = std::getenv("TC_GATHER");
         p->gather_tiles = !(env && std::string(env) == "ray");

@@ -163,6 +163,29 @@ extern "C" tc_status tc_radon1(const float *volume, int n_slices, int n, const f
     return s;
 }
 
+// ---- Beer-Lambert pre-pass + projection -> sinogram reorder ----
+extern "C" tc_status tc_preprocess(const float *proj, const float *flat, const float *dark, int n_angles, int n_slices, int n_det,
+                                   float floor_, float *sinogram, void *stream) {
+    if (!proj || !sinogram || n_angles <= 0 || n_slices <= 0 || n_det <= 0) return fail(TC_EINVAL, "bad argument");
+    if (!(floor_ > 0.f)) return fail(TC_EINVAL, "floor must be positive (it bounds the argument of the logarithm)");
+    const size_t n = (size_t)n_angles * n_slices * n_det, nf = (size_t)n_slices * n_det;
+    const bool dev = is_device_ptr(proj);
+    if (is_device_ptr(sinogram) != dev || (flat && is_device_ptr(flat) != dev) || (dark && is_device_ptr(dark) != dev))
+        return fail(TC_EINVAL, "all arrays must be device pointers or all host pointers");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dev) { launch_preprocess(proj, flat, dark, n_angles, n_slices, n_det, floor_, sinogram, st); return check_launch(); }
+    CallMem mem;
+    float *dp = nullptr, *df = nullptr, *dd = nullptr, *ds = nullptr;
+    CU(mem.alloc(&dp, n)); CU(mem.alloc(&ds, n));
+    CU(cudaMemcpy(dp, proj, n * sizeof(float), cudaMemcpyHostToDevice));
+    if (flat) { CU(mem.alloc(&df, nf)); CU(cudaMemcpy(df, flat, nf * sizeof(float), cudaMemcpyHostToDevice)); }
+    if (dark) { CU(mem.alloc(&dd, nf)); CU(cudaMemcpy(dd, dark, nf * sizeof(float), cudaMemcpyHostToDevice)); }
+    launch_preprocess(dp, df, dd, n_angles, n_slices, n_det, floor_, ds, nullptr);
+    TCS(check_launch());
+    CU(cudaMemcpy(sinogram, ds, n * sizeof(float), cudaMemcpyDeviceToHost));
+    return TC_OK;
+}
+
 // ---- prior test hook ---------------------------------------------------------------------------------
 static tc_status check_prior(const tc_prior *pr) {
     if (!pr) return fail(TC_EINVAL, "null prior");

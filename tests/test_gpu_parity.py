@@ -614,3 +614,20 @@ def test_error_paths_release_device_memory(tc):
     free1 = scenario()
     free2 = scenario()
     assert abs(free2 - free1) <= 4 << 20, (free1, free2)
+
+
+def test_preprocess_vs_oracle(tc):
+    # Beer-Lambert + projection -> sinogram reorder, device and host pointers
+    from oracle import preprocess
+    rng = np.random.default_rng(43)
+    na, S, nd = 13, 5, 96
+    flat = rng.uniform(900, 1100, (S, nd)).astype(np.float32); dark = rng.uniform(5, 15, (S, nd)).astype(np.float32)
+    proj = (rng.uniform(0.05, 1.0, (na, S, nd)) * (flat - dark)[None] + dark[None]).astype(np.float32)
+    proj[3, 2, 10] = dark[2, 10]
+    want = preprocess.preprocess(proj, flat, dark, 1e-5)
+    got_d = _np(tc.preprocess(_cuda(proj), _cuda(flat), _cuda(dark), 1e-5))
+    got_h = tc.preprocess(proj, flat, dark, 1e-5)
+    assert rel_l2(got_d, want) < 1e-6 and np.array_equal(got_d, got_h) and got_d.shape == (S, na, nd)
+    assert rel_l2(_np(tc.preprocess(_cuda(proj))), preprocess.preprocess(proj)) < 1e-6
+    with pytest.raises(tc.TcError):
+        tc.preprocess(_cuda(proj), flat, None)                                 # mixed device / host

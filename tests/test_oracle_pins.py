@@ -498,3 +498,19 @@ def test_mbir_mm_step_decreases_the_surrogate_with_prior():
     assert abs(log[0]["F"] - Fz) < 1e-10 * Fz and Fz <= F0 - 0.5 * np.sum(g * g) ** 2 / den + 1e-9 * F0
     F = [l["F"] for l in log]
     assert all(F[i + 1] <= F[i] for i in range(len(F) - 1)) and all(l["alpha"] > 0 for l in log)
+
+
+def test_preprocess_inverts_beer_lambert_and_reorders():
+    # I = I0 exp(-b) + dark  =>  the pre-pass returns b exactly; every (s, a, u) carries a distinct value, so a wrong
+    # transpose cannot pass; the floor clips dead pixels at -log(floor)
+    from oracle import preprocess
+    na, S, nd = 5, 3, 7
+    s_, a_, u_ = np.meshgrid(np.arange(S), np.arange(na), np.arange(nd), indexing="ij")
+    b = 0.01 + 0.1 * s_ + 0.013 * a_ + 0.0017 * u_                            # sinogram order (S, Na, Nd)
+    rng = np.random.default_rng(42)
+    flat = rng.uniform(900, 1100, (S, nd)); dark = rng.uniform(5, 15, (S, nd))
+    proj = (np.exp(-b) * (flat - dark)[:, None, :] + dark[:, None, :]).transpose(1, 0, 2)      # projection order (Na, S, Nd)
+    assert np.allclose(preprocess.preprocess(proj, flat, dark), b, atol=1e-12)
+    assert np.allclose(preprocess.preprocess(np.exp(-b).transpose(1, 0, 2)), b, atol=1e-12)
+    proj[2, 1, 3] = dark[1, 3]                                                 # a dead pixel
+    assert preprocess.preprocess(proj, flat, dark, floor=1e-4)[1, 2, 3] == -np.log(1e-4)
