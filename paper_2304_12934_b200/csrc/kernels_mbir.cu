@@ -118,30 +118,28 @@ struct PriorK { float inv_sigma, c, p, q; int nonneg; unsigned allow; float wsca
 // q = 2 - p; nonneg: project the candidate on z >= 0; allow: which of the 13 forward offsets belong to the neighbour set (26: all;
 // 10: the 8 in-plane neighbours and the two along z; 6: faces), wscale: renormalises the 1/distance weights to sum 1 over the set
 
-__device__ __forceinline__ float upow(float u, float q) {                                       // u^q, u >= 0: 0 -> 0 (lg2 -> -inf, ex2 -> 0)
-    float r;
-    const float e = q == 0.f ? 0.f : q * __log2f(u);          // p = 2 (q = 0): u^0 = 1 also at u = 0 (0 * -inf would be NaN)
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(e));
-    return r;
-}
+// One evaluation = three MUFU (lg2, ex2, rcp), issued as the bare approximate instructions: u = 0 gives lg2 = -inf, ex2 = 0 (the
+// right limit for q > 0; q = 0, i.e. p = 2, is selected away), and no range fix-ups or branches surround them.
+__device__ __forceinline__ float lg2a(float x) { float r; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float ex2a(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rcpa(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float upow(float u, const PriorK &k) { return k.q == 0.f ? 1.f : ex2a(k.q * lg2a(u)); }     // u^q, u >= 0
 
+// h'(D) = D / sigma^2 * (2c + p u^q) / (c + u^q)^2   (= sign(D)/sigma * u (...) / (...)^2 with u = |D|/sigma)
 __device__ __forceinline__ float dh(float D, const PriorK &k) {
-    const float u = fabsf(D) * k.inv_sigma;
-    const float uq = upow(u, k.q);
-    const float den = k.c + uq;
-    const float v = __fdividef(k.inv_sigma * u * fmaf(k.p, uq, 2.f * k.c), den * den);     // MUFU.RCP + FMUL, 2 ulp
-    return copysignf(v, D);
+    const float uq = upow(fabsf(D) * k.inv_sigma, k);
+    const float r = rcpa(k.c + uq);
+    return (D * r) * (fmaf(k.p, uq, 2.f * k.c) * r) * (k.inv_sigma * k.inv_sigma);
 }
 __device__ __forceinline__ float hval(float D, const PriorK &k) {
     const float u = fabsf(D) * k.inv_sigma;
-    return __fdividef(u * u, k.c + upow(u, k.q));
+    return u * u * rcpa(k.c + upow(u, k));
 }
 // h'(D) / D = (2c + p u^q) / (sigma^2 (c + u^q)^2): the curvature of the quadratic surrogate of h at D (finite at D = 0: 2 / (c sigma^2))
 __device__ __forceinline__ float hcurv(float D, const PriorK &k) {
-    const float u = fabsf(D) * k.inv_sigma;
-    const float uq = upow(u, k.q);
-    const float den = k.c + uq;
-    return __fdividef(k.inv_sigma * k.inv_sigma * fmaf(k.p, uq, 2.f * k.c), den * den);
+    const float uq = upow(fabsf(D) * k.inv_sigma, k);
+    const float r = rcpa(k.c + uq);
+    return (fmaf(k.p, uq, 2.f * k.c) * r) * (r * (k.inv_sigma * k.inv_sigma));
 }
 
 // w_mn = (1/dist) / (6 + 12/sqrt2 + 8/sqrt3)  (reading G10)
@@ -215,16 +213,16 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__
 #pragma unroll
                 for (int dx = -1; dx <= 1; ++dx) {
                     if (dy == 0 && dx <= 0) continue;
-                    float dv = 0.f;
-                    if (mk >> o & 1) dv = wgt(0, dy, dx) * dh(c_cur - vc[dy * 34 + dx], pk);
+                    const float ev = wgt(0, dy, dx) * dh(c_cur - vc[dy * 34 + dx], pk);       // evaluated unconditionally (a NaN halo is selected away)
+                    const float dv = (mk >> o & 1) ? ev : 0.f;
                     din[o][hy][hx] = dv; acc += dv; ++o;
                 }
 #pragma unroll
             for (int dy = -1; dy <= 1; ++dy)
 #pragma unroll
                 for (int dx = -1; dx <= 1; ++dx) {
-                    float dv = 0.f;
-                    if (mk >> o & 1) dv = wgt(1, dy, dx) * dh(c_cur - vu[dy * 34 + dx], pk);
+                    const float ev = wgt(1, dy, dx) * dh(c_cur - vu[dy * 34 + dx], pk);
+                    const float dv = (mk >> o & 1) ? ev : 0.f;
                     dup[zz & 1][o - 4][hy][hx] = dv; acc += dv; ++o;
                 }
         }
@@ -322,9 +320,11 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *_
 #pragma unroll
                     for (int dx = -1; dx <= 1; ++dx) {
                         if (dy == 0 && dx <= 0) continue;
-                        if (mk >> o & 1) {
-                            if (CURV) { const float dg = g_cur - gc[dy * 34 + dx]; acc = fmaf(wgt(0, dy, dx) * hcurv(c_cur - vc[dy * 34 + dx], pk), dg * dg, acc); }
-                            else acc = fmaf(wgt(0, dy, dx), hval(c_cur - vc[dy * 34 + dx], pk), acc);
+                        {
+                            float ev;
+                            if (CURV) { const float dg = g_cur - gc[dy * 34 + dx]; ev = wgt(0, dy, dx) * hcurv(c_cur - vc[dy * 34 + dx], pk) * (dg * dg); }
+                            else ev = wgt(0, dy, dx) * hval(c_cur - vc[dy * 34 + dx], pk);
+                            acc += (mk >> o & 1) ? ev : 0.f;
                         }
                         ++o;
                     }
@@ -332,9 +332,11 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *_
                 for (int dy = -1; dy <= 1; ++dy)
 #pragma unroll
                     for (int dx = -1; dx <= 1; ++dx) {
-                        if (mk >> o & 1) {
-                            if (CURV) { const float dg = g_cur - gu[dy * 34 + dx]; acc = fmaf(wgt(1, dy, dx) * hcurv(c_cur - vu[dy * 34 + dx], pk), dg * dg, acc); }
-                            else acc = fmaf(wgt(1, dy, dx), hval(c_cur - vu[dy * 34 + dx], pk), acc);
+                        {
+                            float ev;
+                            if (CURV) { const float dg = g_cur - gu[dy * 34 + dx]; ev = wgt(1, dy, dx) * hcurv(c_cur - vu[dy * 34 + dx], pk) * (dg * dg); }
+                            else ev = wgt(1, dy, dx) * hval(c_cur - vu[dy * 34 + dx], pk);
+                            acc += (mk >> o & 1) ? ev : 0.f;
                         }
                         ++o;
                     }
