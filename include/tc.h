@@ -102,6 +102,25 @@ tc_status tc_preprocess(const float *proj, const float *flat, const float *dark,
 tc_status tc_mbir(tc_plan *plan, const float *sinogram, int n_slices, const tc_prior *prior, int iters,
                   float *volume, tc_iter_log *log, void *cuda_stream);
 
+/* z-sharded MBIR (the paper's level-1 partition: one contiguous range of slices per GPU).  Forward and adjoint are
+ * slice-wise, so the ranks only meet in the prior (one halo slice of the candidate towards each z-neighbour per iteration)
+ * and in the three scalars of the accept test.  The library does the arithmetic; the caller supplies the transport:
+ *   exchange(ctx): deliver this rank's send_down to the lower rank's recv_up and send_up to the upper rank's recv_down (n*n floats
+ *                  each).  The send buffers are complete when it is called; the recv buffers must be complete when it returns.
+ *   allreduce(ctx, vals, n): in-place sum over all ranks of n doubles in HOST memory (same result on every rank).
+ * Both return 0 on success.  send_ / recv_ buffers are DEVICE memory owned by the caller; a rank at the bottom (top) of the volume
+ * passes NULL for the down (up) pair.  tc_mbir_sharded(sinogram, volume: DEVICE, this rank's n_slices) is tc_mbir on the rank's
+ * range; prior->L must be given (> 0, the same everywhere) and every rank must make the same calls.  The iterate sequence equals
+ * the unsharded one up to the float64 summation order of the objective. */
+typedef struct {
+    void *ctx;
+    int (*exchange)(void *ctx);
+    int (*allreduce)(void *ctx, double *vals, int n);
+    float *send_down, *send_up, *recv_down, *recv_up;
+} tc_comm;
+tc_status tc_mbir_sharded(tc_plan *plan, const float *sinogram, int n_slices, const tc_prior *prior, int iters, float *volume,
+                          tc_iter_log *log, const tc_comm *comm, void *cuda_stream);
+
 /* lambda_hat = ||A^T A v|| / ||v|| after `iters` power iterations on one slice from v = ones. */
 tc_status tc_power_iteration(tc_plan *plan, int iters, double *lambda_hat);
 

@@ -39,6 +39,15 @@ class tc_sched_stats(ctypes.Structure):
                 ("d2h_bytes", ctypes.c_longlong), ("n_slabs", ctypes.c_int), ("setup_s", ctypes.c_double), ("handover_s", ctypes.c_double)]
 
 
+EXCHANGE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p)
+ALLREDUCE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_int)
+
+
+class tc_comm(ctypes.Structure):
+    _fields_ = [("ctx", ctypes.c_void_p), ("exchange", EXCHANGE_FN), ("allreduce", ALLREDUCE_FN),
+                ("send_down", ctypes.c_void_p), ("send_up", ctypes.c_void_p), ("recv_down", ctypes.c_void_p), ("recv_up", ctypes.c_void_p)]
+
+
 _vp, _ci = ctypes.c_void_p, ctypes.c_int
 lib.tc_plan_create.argtypes = [ctypes.POINTER(tc_geom), _ci, ctypes.POINTER(_vp)]
 lib.tc_plan_destroy.argtypes = [_vp]
@@ -46,6 +55,7 @@ lib.tc_radon.argtypes = [_vp, _vp, _ci, _vp, _vp]
 lib.tc_backproject.argtypes = [_vp, _vp, _ci, _vp, _vp]
 lib.tc_fbp.argtypes = [_vp, _vp, _ci, _ci, _vp, _vp]
 lib.tc_mbir.argtypes = [_vp, _vp, _ci, ctypes.POINTER(tc_prior), _ci, _vp, ctypes.POINTER(tc_iter_log), _vp]
+lib.tc_mbir_sharded.argtypes = [_vp, _vp, _ci, ctypes.POINTER(tc_prior), _ci, _vp, ctypes.POINTER(tc_iter_log), ctypes.POINTER(tc_comm), _vp]
 lib.tc_power_iteration.argtypes = [_vp, _ci, ctypes.POINTER(ctypes.c_double)]
 lib.tc_prior_eval.argtypes = [_vp, _ci, _ci, ctypes.POINTER(tc_prior), _vp, ctypes.POINTER(ctypes.c_double)]
 lib.tc_radon1.argtypes = [_vp, _ci, _ci, ctypes.POINTER(ctypes.c_float), _ci, _ci, ctypes.c_float, _vp]
@@ -59,7 +69,7 @@ lib.tc_host_alloc.argtypes = [ctypes.c_size_t, ctypes.POINTER(_vp)]
 lib.tc_host_free.argtypes = [_vp]
 lib.tc_last_error.restype = ctypes.c_char_p
 for _f in ("tc_plan_create", "tc_plan_destroy", "tc_radon", "tc_backproject", "tc_fbp", "tc_mbir", "tc_power_iteration",
-           "tc_prior_eval", "tc_radon1", "tc_last_sched_stats", "tc_profile", "tc_profile_read", "tc_host_alloc", "tc_host_free", "tc_preprocess"):
+           "tc_prior_eval", "tc_radon1", "tc_last_sched_stats", "tc_profile", "tc_profile_read", "tc_host_alloc", "tc_host_free", "tc_preprocess", "tc_mbir_sharded"):
     getattr(lib, _f).restype = _ci
 
 
@@ -146,6 +156,39 @@ class Plan:
         out = _like(sinogram, (S, self.n, self.n)) if out is None else out
         log = (tc_iter_log * max(iters, 1))()
         _check(lib.tc_mbir(self._h, _ptr(sinogram), S, ctypes.byref(prior), int(iters), _ptr(out), log, _stream(sinogram)))
+        recs = [dict(F=l.F, data=l.data, prior=l.prior, margin=l.margin, dot=l.dot, beta=l.beta, accepted=l.accepted, restarted=l.restarted, alpha=l.alpha)
+                for l in log[:iters]]
+        return out, recs
+
+    def mbir_sharded(self, sinogram, prior, iters, comm, out=None):
+        """tc_mbir_sharded on this rank's slices; `comm` has the attributes of shard.TorchComm (exchange(), allreduce(list) -> list,
+        send_down / send_up / recv_down / recv_up: device tensors or None)."""
+        S = sinogram.shape[0]
+        assert sinogram.is_cuda and tuple(sinogram.shape) == (S, self.n_angles, self.n_det)
+        out = _like(sinogram, (S, self.n, self.n)) if out is None else out
+        log = (tc_iter_log * max(iters, 1))()
+        errs = []
+
+        def _ex(_ctx):
+            try:
+                comm.exchange(); return 0
+            except Exception as e:                                   # an exception must not unwind through the C frames
+                errs.append(e); return 1
+
+        def _ar(_ctx, vals, n):
+            try:
+                res = comm.allreduce([vals[i] for i in range(n)])
+                for i in range(n):
+                    vals[i] = res[i]
+                return 0
+            except Exception as e:
+                errs.append(e); return 1
+        ptr = lambda t: None if t is None else t.data_ptr()
+        c = tc_comm(None, EXCHANGE_FN(_ex), ALLREDUCE_FN(_ar), ptr(comm.send_down), ptr(comm.send_up), ptr(comm.recv_down), ptr(comm.recv_up))
+        st = lib.tc_mbir_sharded(self._h, _ptr(sinogram), S, ctypes.byref(prior), int(iters), _ptr(out), log, ctypes.byref(c), _stream(sinogram))
+        if errs:
+            raise errs[0]
+        _check(st)
         recs = [dict(F=l.F, data=l.data, prior=l.prior, margin=l.margin, dot=l.dot, beta=l.beta, accepted=l.accepted, restarted=l.restarted, alpha=l.alpha)
                 for l in log[:iters]]
         return out, recs

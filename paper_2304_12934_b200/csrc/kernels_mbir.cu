@@ -153,26 +153,30 @@ __device__ __forceinline__ float wgt(int dz, int dy, int dx) {
 
 // M2 + M3, pair-sharing form.  h' is odd, so the pair {m, n} gives +d to m and -d to n with d = w h'(y_m - y_n): every pair
 // is evaluated ONCE (13 "forward" pairs per voxel instead of 26; the evaluation costs three MUFU and bounds the kernel).
-// A CTA owns a 32 x 8 tile with a one-voxel halo ring (34 x 10 = 340 of its 352 threads, one thread per column) and marches
+// A CTA owns a 32 x PM_TY tile with a one-voxel halo ring (34 x (PM_TY + 2) threads, one per column; PM_TY = 12: 476 of 480) and marches
 // through a chunk of slices: at slice s a thread evaluates its 4 in-plane forward pairs and its 9 pairs with slice s + 1,
 // leaves d in shared memory for the partner (the in-plane ones are picked up in the same step, the 9 others in the next
 // step), and the interior threads write g and z.  One warm-up step below the chunk supplies the first slice's incoming pairs.
 constexpr int PM_ZC = 16;        // output slices per chunk
-constexpr int PM_THREADS = 352;
+#ifndef PM_TY
+#define PM_TY 12
+#endif
+constexpr int PM_HY = PM_TY + 2, PM_LIVE = 34 * PM_HY;      // tile rows (PM_TY) plus the halo ring; threads that hold a column
+constexpr int PM_THREADS = (PM_LIVE + 31) / 32 * 32;
 
 // The input is y = x + beta (x - x-), formed while loading when xm != nullptr (M1 fused: y never reaches HBM in the in-core loop).
 template <bool STEP, bool EXTRAP>
 __global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__restrict__ y, const float *__restrict__ xm, float beta,
                                                                  const float *atr, PriorK pk, float lambda,
                                                                  float invL, float *g, float *__restrict__ z, int S, int n, int s_first, int n_out) {
-    __shared__ float val[2][10][34];
-    __shared__ float din[4][10][34];
-    __shared__ float dup[2][9][10][34];
+    __shared__ float val[2][PM_HY][34];
+    __shared__ float din[4][PM_HY][34];
+    __shared__ float dup[2][9][PM_HY][34];
     const int t = threadIdx.x, hx = t % 34, hy = t / 34;
-    const bool live = t < 340;
-    const int gx = blockIdx.x * 32 + hx - 1, gy = blockIdx.y * 8 + hy - 1;
+    const bool live = t < PM_LIVE;
+    const int gx = blockIdx.x * 32 + hx - 1, gy = blockIdx.y * PM_TY + hy - 1;
     const bool inplane = live && gx >= 0 && gx < n && gy >= 0 && gy < n;
-    const bool core = hx >= 1 && hx <= 32 && hy >= 1 && hy <= 8;
+    const bool core = hx >= 1 && hx <= 32 && hy >= 1 && hy <= PM_TY;
     const bool interior = inplane && core;
     const int zlo = s_first + blockIdx.z * PM_ZC, zhi = min(zlo + PM_ZC, s_first + n_out);
     const int zstart = zlo > 0 ? zlo - 1 : 0;
@@ -188,8 +192,8 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__
                 for (int dx = -1; dx <= 1; ++dx) {
                     if (dz == 0 && (dy < 0 || (dy == 0 && dx <= 0))) continue;
                     const int ny = hy + dy, nx = hx + dx, px = gx + dx, py = gy + dy;
-                    const bool pcore = nx >= 1 && nx <= 32 && ny >= 1 && ny <= 8;
-                    if (inplane && ny >= 0 && ny < 10 && nx >= 0 && nx < 34 && px >= 0 && px < n && py >= 0 && py < n && (core || pcore)) mask |= 1u << o;
+                    const bool pcore = nx >= 1 && nx <= 32 && ny >= 1 && ny <= PM_TY;
+                    if (inplane && ny >= 0 && ny < PM_HY && nx >= 0 && nx < 34 && px >= 0 && px < n && py >= 0 && py < n && (core || pcore)) mask |= 1u << o;
                     ++o;
                 }
         mask &= pk.allow;
@@ -262,20 +266,20 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__
 template <bool CURV>
 __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *__restrict__ zv, const float *__restrict__ xm, float beta,
                                                                   const float *__restrict__ gdir, PriorK pk, double *partials, int S, int n, int S_own) {
-    __shared__ float val[2][10][34];
-    __shared__ float gval[CURV ? 2 : 1][CURV ? 10 : 1][CURV ? 34 : 1];
+    __shared__ float val[2][PM_HY][34];
+    __shared__ float gval[CURV ? 2 : 1][CURV ? PM_HY : 1][CURV ? 34 : 1];
     __shared__ double red[PM_THREADS / 32];
     const int t = threadIdx.x, hx = t % 34, hy = t / 34;
-    const bool live = t < 340;
-    const bool core = hx >= 1 && hx <= 32 && hy >= 1 && hy <= 8;
-    const int ntx = (n + 31) / 32, nty = (n + 7) / 8, nch = (S_own + PM_ZC - 1) / PM_ZC;
+    const bool live = t < PM_LIVE;
+    const bool core = hx >= 1 && hx <= 32 && hy >= 1 && hy <= PM_TY;
+    const int ntx = (n + 31) / 32, nty = (n + PM_TY - 1) / PM_TY, nch = (S_own + PM_ZC - 1) / PM_ZC;
     const long long nitems = (long long)ntx * nty * nch;
     const size_t plane = (size_t)n * n;
     auto ldv = [&](size_t i) { const float a = zv[i]; return CURV ? fmaf(beta, a - xm[i], a) : a; };
     double sum = 0.0;
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int ch = (int)(item / (ntx * nty)), r = (int)(item % (ntx * nty));
-        const int gx = (r % ntx) * 32 + hx - 1, gy = (r / ntx) * 8 + hy - 1;
+        const int gx = (r % ntx) * 32 + hx - 1, gy = (r / ntx) * PM_TY + hy - 1;
         const bool inplane = live && gx >= 0 && gx < n && gy >= 0 && gy < n;
         unsigned mask = 0;
         {
@@ -379,7 +383,7 @@ void launch_residual(const float *Ax, const float *Axm, const float *b, float be
 void launch_update(const float *x, const float *xm, float beta, const float *atr, PriorDev pr, float invL, float *g, float *z, int S, int n,
                    cudaStream_t st, int s_first, int n_out) {
     if (n_out < 0) n_out = S - s_first;
-    dim3 gr((n + 31) / 32, (n + 7) / 8, (n_out + PM_ZC - 1) / PM_ZC);
+    dim3 gr((n + 31) / 32, (n + PM_TY - 1) / PM_TY, (n_out + PM_ZC - 1) / PM_ZC);
     const PriorK k = mk(pr);
     if (xm) {
         if (z) k_prior_grad_march<true, true><<<gr, PM_THREADS, 0, st>>>(x, xm, beta, atr, k, pr.lambda, invL, g, z, S, n, s_first, n_out);

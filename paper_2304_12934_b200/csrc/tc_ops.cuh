@@ -266,17 +266,22 @@ static tc_status mbir_streamed(tc_plan *p, const float *hb, int S, const tc_prio
 // A y the same way.  A rejected candidate changes nothing but t (the next step has beta = 0, so x- is not even read).
 constexpr int AX_REFRESH = 50;
 
+// z-sharded form (comm != nullptr; P:L133 level-1 partition): this rank owns S consecutive slices of a taller volume.
+// A and A^T are slice-wise, so only the prior couples the ranks: the volume arrays carry one halo slice towards each neighbour
+// (lo / hi), the candidate's boundary slices are exchanged once per iteration (x and x- inherit their halos through the pointer
+// rotation), and the terms of the objective are summed over ranks before the accept test, so every rank takes the same decision.
 static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc_prior *pr, int iters, float *volume, tc_iter_log *log,
-                              double L, cudaStream_t st, bool dev_b, bool dev_v, bool *retry_streamed) {
+                              double L, cudaStream_t st, bool dev_b, bool dev_v, bool *retry_streamed, const tc_comm *comm = nullptr) {
     const DevPlan &d = p->d;
     const size_t vps = (size_t)d.n * d.n, sps = (size_t)d.na * d.nd;
-    const size_t nv = (size_t)S * vps, ns = (size_t)S * sps;
+    const int lo = comm && comm->send_down ? 1 : 0, hi = comm && comm->send_up ? 1 : 0, Sx = S + lo + hi;
+    const size_t nv = (size_t)S * vps, ns = (size_t)S * sps, nvx = (size_t)Sx * vps;
     *retry_streamed = false;
     int slab; TCS(ensure_scratch(p, S, &slab, 16));           // at most 16 groups of FFT scratch: the state below needs the memory
     CallMem mem;
     float *vb[4] = {nullptr}, *sb[5] = {nullptr};
     bool ok = true;
-    for (int i = 0; i < 4 && ok; ++i) ok = mem.alloc(&vb[i], nv) == cudaSuccess;
+    for (int i = 0; i < 4 && ok; ++i) ok = mem.alloc(&vb[i], nvx) == cudaSuccess;
     for (int i = 0; i < 5 && ok; ++i) {
         if (i == 4 && dev_b) { sb[4] = const_cast<float *>(sinogram); continue; }
         ok = mem.alloc(&sb[i], ns) == cudaSuccess;
@@ -286,10 +291,14 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
         return fail(TC_ENOMEM, "tc_mbir: the in-core working set (4 volumes + 5 sinograms) does not fit in device memory; "
                                "pass host pointers to stream the problem");
     }
-    float *x = vb[0], *xm = vb[1], *z = vb[2], *gv = vb[3];
+    // xe, xme, ze, ge: arrays of Sx slices (halo, core, halo); x, xm, z, gv: their core parts
+    float *xe = vb[0], *xme = vb[1], *ze = vb[2], *ge = vb[3];
+    const size_t co = (size_t)lo * vps;
+    float *x = xe + co, *xm = xme + co, *z = ze + co, *gv = ge + co;
     float *Ax = sb[0], *Axm = sb[1], *Az = sb[2], *r = sb[3], *b = sb[4];
     if (!dev_b) CU(cudaMemcpyAsync(b, sinogram, ns * sizeof(float), cudaMemcpyHostToDevice, st));
-    CU(cudaMemsetAsync(x, 0, nv * sizeof(float), st)); CU(cudaMemsetAsync(xm, 0, nv * sizeof(float), st));
+    CU(cudaMemsetAsync(xe, 0, nvx * sizeof(float), st)); CU(cudaMemsetAsync(xme, 0, nvx * sizeof(float), st));
+    CU(cudaMemsetAsync(ze, 0, nvx * sizeof(float), st));
     CU(cudaMemsetAsync(Ax, 0, ns * sizeof(float), st)); CU(cudaMemsetAsync(Axm, 0, ns * sizeof(float), st));
     CU(cudaMemsetAsync(p->acc, 0, 16 * sizeof(double), st));
     launch_sumsq(b, ns, p->acc, 2, st);
@@ -297,6 +306,7 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
     CU(cudaMemcpyAsync(h, p->acc, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
     TCS(check_launch());
+    if (comm && comm->allreduce(comm->ctx, h + 2, 1) != 0) return fail(TC_ECUDA, "tc_mbir_sharded: allreduce callback failed");
     double Fx = 0.5 * h[2], t = 1.0;
     const PriorDev pd = prior_dev(pr);
     const float invL = (float)(1.0 / L);
@@ -329,7 +339,7 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
             alpha = den > 0.0 ? (float)(h[4] / den) : invL;
             launch_step(x, xm, beta, gv, alpha, pd.nonneg, z, nv, st);                        // z = y - alpha g (projected if nonneg)
         } else {
-            launch_update(x, xm, beta, gv, pd, invL, gv, z, S, d.n, st);                      // M2 + M3: g, z = y - g / L
+            launch_update(xe, xme, beta, ge, pd, invL, ge, ze, Sx, d.n, st, lo, S);           // M2 + M3: g, z = y - g / L on the core
         }
         if (pd.nonneg) {                                                  // projected candidate: z is not linear in g, so A z itself
             slabbed(forward_slab, z, vps, r, sps);
@@ -338,17 +348,27 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
             if (!pr->mm_step) slabbed(forward_slab, gv, vps, r, sps);     // A g
             launch_candidate_sino(Ax, Axm, r, b, beta, alpha, Az, p->acc, ns, st);            // M4: Az = A y - alpha A g
         }
-        launch_prior(z, pd, nullptr, p->acc, S, d.n, st);
+        if (comm) {                                                       // the candidate's boundary slices go to the neighbours' halos
+            if (lo) CU(cudaMemcpyAsync(comm->send_down, z, vps * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            if (hi) CU(cudaMemcpyAsync(comm->send_up, z + (size_t)(S - 1) * vps, vps * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            CU(cudaStreamSynchronize(st));
+            if (comm->exchange(comm->ctx) != 0) return fail(TC_ECUDA, "tc_mbir_sharded: halo exchange callback failed");
+            if (lo) CU(cudaMemcpyAsync(ze, comm->recv_down, vps * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            if (hi) CU(cudaMemcpyAsync(ze + (size_t)(Sx - 1) * vps, comm->recv_up, vps * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        }
+        launch_prior(z, pd, nullptr, p->acc, S + hi, d.n, st, S);         // pairs are owned by their lower slice: the core's, up to the upper halo
         if (pr->grad_restart) launch_dot_gzx(gv, z, x, nv, p->acc, 3, st);
         CU(cudaMemcpyAsync(h, p->acc, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
         TCS(check_launch());
+        if (comm && comm->allreduce(comm->ctx, h, 4) != 0) return fail(TC_ECUDA, "tc_mbir_sharded: allreduce callback failed");
         const double Fz = h[0] + (double)pr->lambda * h[1];
         const double margin = (Fx - Fz) / Fx;
         const bool accept = Fz <= Fx;                                     // M5
         const bool restarted = pr->grad_restart && accept && h[3] > 0.0;
         if (accept) {
-            float *ox = xm; xm = x; x = z; z = ox;
+            float *oe = xme; xme = xe; xe = ze; ze = oe;
+            x = xe + co; xm = xme + co; z = ze + co;
             float *oa = Axm; Axm = Ax; Ax = Az; Az = oa;
             Fx = Fz; t = restarted ? 1.0 : tp;
         } else {
@@ -398,4 +418,22 @@ extern "C" tc_status tc_mbir(tc_plan *p, const float *sinogram, int S, const tc_
     const tc_status s = mbir_in_core(p, sinogram, S, pr, iters, volume, log, L, (cudaStream_t)stream, dev_b, dev_v, &retry);
     if (s == TC_ENOMEM && retry) return stream_it();                      // the estimate was wrong (fragmentation, other tenants): stream instead
     return s;
+}
+
+// ---- z-sharded MBIR: one rank of a volume partitioned along the rotation axis ----
+extern "C" tc_status tc_mbir_sharded(tc_plan *p, const float *sinogram, int S, const tc_prior *pr, int iters, float *volume,
+                                     tc_iter_log *log, const tc_comm *comm, void *stream) {
+    if (!p || !sinogram || !volume || !comm) return fail(TC_EINVAL, "null argument");
+    if (S <= 0 || iters < 0) return fail(TC_EINVAL, "n_slices must be positive, iters non-negative");
+    if (!comm->exchange || !comm->allreduce) return fail(TC_EINVAL, "tc_comm: exchange and allreduce callbacks are required");
+    if ((comm->send_down == nullptr) != (comm->recv_down == nullptr) || (comm->send_up == nullptr) != (comm->recv_up == nullptr))
+        return fail(TC_EINVAL, "tc_comm: send / recv buffers must come in pairs");
+    TCS(check_prior(pr));
+    if (pr->mm_step) return fail(TC_EUNSUPPORTED, "tc_mbir_sharded: mm_step is not available");
+    if (!(pr->L > 0.f)) return fail(TC_EINVAL, "tc_mbir_sharded: pass the step constant L (the same on every rank)");
+    if (!is_device_ptr(sinogram) || !is_device_ptr(volume)) return fail(TC_EINVAL, "tc_mbir_sharded: device pointers only");
+    for (const float *q : {comm->send_down, comm->recv_down, comm->send_up, comm->recv_up})
+        if (q && !is_device_ptr(q)) return fail(TC_EINVAL, "tc_comm: halo buffers must be device memory");
+    bool retry = false;
+    return mbir_in_core(p, sinogram, S, pr, iters, volume, log, (double)pr->L, (cudaStream_t)stream, true, true, &retry, comm);
 }

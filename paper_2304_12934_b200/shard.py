@@ -1,6 +1,11 @@
-"""z-sharding for N > 1 GPUs: the path partitions by slice -- forward and adjoint are independent
-per slice, so ranks take contiguous z-ranges with no data-path collective ("weak" replicas of the slab pipeline).
-MBIR's 26-neighbour prior would need a one-slice halo exchange per iteration; that is SURVEY 8(f) #3, not built."""
+"""z-sharding for N > 1 GPUs: the path partitions by slice.
+
+Forward and adjoint are independent per slice, so ranks take contiguous z-ranges with no data-path collective (bench.py --gpus N:
+"weak" replicas of the slab pipeline).  MBIR couples slices only through the prior's neighbourhood and three global scalars:
+`TorchComm` is the transport `tc_mbir_sharded` asks for (include/tc.h: tc_comm) -- one halo slice to each z-neighbour and one
+all-reduce of four doubles per iteration -- on torch.distributed (NCCL point-to-point over NVLink on GPUs; gloo on CPU for tests).
+No arithmetic of the method lives here.
+"""
 
 
 def shard_slices(n_slices, rank, world):
@@ -19,3 +24,35 @@ def max_over_ranks(seconds, device="cuda"):
     t = torch.tensor([float(seconds)], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+class TorchComm:
+    """Halo exchange and scalar all-reduce between z-neighbours rank - 1 (down) and rank + 1 (up) of the default process group.
+    send_down / send_up / recv_down / recv_up are (n, n) float32 tensors on `device`, None where there is no neighbour."""
+
+    def __init__(self, n, device="cuda", rank=None, world=None):
+        import torch, torch.distributed as dist
+        self.dist, self.torch = dist, torch
+        self.rank = dist.get_rank() if rank is None else rank
+        self.world = dist.get_world_size() if world is None else world
+        self.device = device
+        mk = lambda: torch.zeros((n, n), dtype=torch.float32, device=device)
+        self.send_down, self.recv_down = (mk(), mk()) if self.rank > 0 else (None, None)
+        self.send_up, self.recv_up = (mk(), mk()) if self.rank < self.world - 1 else (None, None)
+
+    def exchange(self):
+        d, ops = self.dist, []
+        if self.rank > 0:
+            ops += [d.P2POp(d.isend, self.send_down, self.rank - 1), d.P2POp(d.irecv, self.recv_down, self.rank - 1)]
+        if self.rank < self.world - 1:
+            ops += [d.P2POp(d.isend, self.send_up, self.rank + 1), d.P2POp(d.irecv, self.recv_up, self.rank + 1)]
+        if ops:
+            for r in d.batch_isend_irecv(ops):
+                r.wait()
+        if self.device != "cpu":
+            self.torch.cuda.synchronize()
+
+    def allreduce(self, vals):
+        t = self.torch.tensor(list(vals), dtype=self.torch.float64, device=self.device)
+        self.dist.all_reduce(t)
+        return t.tolist()

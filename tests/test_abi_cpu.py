@@ -16,7 +16,8 @@ def test_library_exports_every_declared_symbol():
     hdr = open(os.path.join(ROOT, "include", "tc.h")).read()
     names = set(re.findall(r"\b(tc_[a-z0-9_]+)\s*\(", hdr))
     assert {"tc_plan_create", "tc_plan_destroy", "tc_radon", "tc_backproject", "tc_mbir", "tc_radon1",
-            "tc_power_iteration", "tc_prior_eval", "tc_last_error", "tc_launch_count", "tc_last_sched_stats", "tc_fbp"} <= names
+            "tc_power_iteration", "tc_prior_eval", "tc_last_error", "tc_launch_count", "tc_last_sched_stats", "tc_fbp",
+            "tc_mbir_sharded", "tc_preprocess", "tc_host_alloc", "tc_host_free"} <= names
     lib = _lib()
     for n in names:
         assert hasattr(lib, n), n
@@ -69,13 +70,22 @@ def test_shard_slices_partition():
 _WORKER = r'''
 import os, sys, torch, torch.distributed as dist
 sys.path.insert(0, sys.argv[1])
-from paper_2304_12934_b200.shard import shard_slices, max_over_ranks
+from paper_2304_12934_b200.shard import shard_slices, max_over_ranks, TorchComm
 dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%s" % sys.argv[2], rank=int(sys.argv[3]), world_size=2)
 r = dist.get_rank()
 lo, hi = shard_slices(20, r, 2)
 t = max_over_ranks(1.0 + r, device="cpu")
 tot = torch.tensor([float(hi - lo)]); dist.all_reduce(tot)
 assert t == 2.0 and tot.item() == 20.0, (t, tot)
+# the transport of tc_mbir_sharded (include/tc.h: tc_comm): halo slices to the z-neighbours, sum of the objective's terms
+c = TorchComm(4, device="cpu")
+assert (c.send_down is None) == (r == 0) and (c.send_up is None) == (r == 1)
+if r == 0: c.send_up.fill_(10.0)
+else: c.send_down.fill_(21.0)
+c.exchange()
+if r == 0: assert torch.all(c.recv_up == 21.0)
+else: assert torch.all(c.recv_down == 10.0)
+assert c.allreduce([1.0 + r, 0.5, -2.0 * r, 0.0]) == [3.0, 1.0, -2.0, 0.0]
 dist.barrier(); dist.destroy_process_group()
 '''
 

@@ -631,3 +631,72 @@ def test_preprocess_vs_oracle(tc):
     assert rel_l2(_np(tc.preprocess(_cuda(proj))), preprocess.preprocess(proj)) < 1e-6
     with pytest.raises(tc.TcError):
         tc.preprocess(_cuda(proj), flat, None)                                 # mixed device / host
+
+
+@pytest.mark.parametrize("name", ["alternating", "plain"])
+def test_mbir_z_sharded_two_ranks_on_one_gpu(tc, name):
+    # tc_mbir_sharded.  Two "ranks" = two host threads of this process, each with its own plan and its own
+    # z-range, meeting only on the host (a threading.Barrier inside the transport callbacks): no kernel waits for another one.
+    # The result must equal the unsharded run (and the oracle), rejected candidates included.
+    import threading, torch
+    if name == "alternating":
+        b, ang, n, centre, pr, L, iters, xo, logo, _ = _reject_case("alternating")
+    else:
+        from paper_2304_12934_b200 import inputs
+        from oracle import nufft, mbir
+        S, n, na, centre, iters = 19, 64, 24, 32.0, 6
+        ang = inputs.angles_uniform(na); a64 = ang.astype(np.float64)
+        b = (nufft.radon_nufft(inputs.volume_cfg2(S=S, n=n), a64, n, centre) + 0.01 * np.random.default_rng(18).standard_normal((S, na, n))).astype(np.float32)
+        pr = (P, SIG, C, 1.0)
+        L, _ = mbir.lipschitz(n, a64, n, centre, *pr)
+        xo, logo = mbir.mbir(b, a64, n, centre, *pr, L, iters)
+    S = b.shape[0]
+    prior = tc.prior_params(*pr, L)
+    plan = tc.Plan(n, b.shape[-1], ang, centre)
+    x_ref, log_ref = plan.mbir(_cuda(b), prior, iters); x_ref = _np(x_ref); plan.close()
+    cut = S // 2 + 1
+    bounds = [(0, cut), (cut, S)]
+    bar = threading.Barrier(2)
+    shared = {"vals": [None, None]}
+
+    class LocalComm:
+        def __init__(self, r):
+            self.r = r
+            mk = lambda: torch.zeros((n, n), dtype=torch.float32, device="cuda")
+            self.send_down, self.recv_down = (mk(), mk()) if r == 1 else (None, None)
+            self.send_up, self.recv_up = (mk(), mk()) if r == 0 else (None, None)
+
+        def exchange(self):
+            bar.wait()
+            other = comms[1 - self.r]
+            if self.r == 0: self.recv_up.copy_(other.send_down)
+            else: self.recv_down.copy_(other.send_up)
+            torch.cuda.synchronize()
+            bar.wait()
+
+        def allreduce(self, vals):
+            shared["vals"][self.r] = list(vals)
+            bar.wait()
+            out = [shared["vals"][0][i] + shared["vals"][1][i] for i in range(len(vals))]
+            bar.wait()
+            return out
+
+    comms = [LocalComm(0), LocalComm(1)]
+    res, errs = [None, None], []
+
+    def rank(r):
+        try:
+            lo, hi = bounds[r]
+            pl = tc.Plan(n, b.shape[-1], ang, centre)
+            x, log = pl.mbir_sharded(_cuda(b[lo:hi]), prior, iters, comms[r])
+            res[r] = (_np(x), log); pl.close()
+        except Exception as e:
+            errs.append(e); bar.abort()
+    th = [threading.Thread(target=rank, args=(r,)) for r in range(2)]
+    [t.start() for t in th]; [t.join(timeout=300) for t in th]
+    assert not errs, errs
+    x = np.concatenate([res[0][0], res[1][0]])
+    assert [l["accepted"] for l in res[0][1]] == [l["accepted"] for l in res[1][1]] == [l["accepted"] for l in log_ref] == [l["accepted"] for l in logo]
+    assert rel_l2(x, x_ref) <= 1e-6 and rel_l2(x, xo) < TOL_MBIR
+    for l0, l1, lr in zip(res[0][1], res[1][1], log_ref):
+        assert l0["F"] == l1["F"] and abs(l0["F"] - lr["F"]) <= 1e-9 * abs(lr["F"])
