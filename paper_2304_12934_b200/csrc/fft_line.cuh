@@ -30,6 +30,7 @@ __device__ __forceinline__ int pcell(int c) { return c + (c >> 4); }
 template <int PL_, int N_, int TWS_, int... Rs> struct SCfg {
     static constexpr bool is_static = true;
     static constexpr bool PM_LAST = false;
+    static constexpr int GROUP_THREADS = 0;
     static constexpr int PL = PL_;
     static constexpr int SLOTS = N_ / 16 < LINE_SLOTS ? (N_ / 16 < 32 ? 32 : N_ / 16) : LINE_SLOTS;   // one radix-16 task per thread when the line is short
     static constexpr int NP = sizeof...(Rs);
@@ -41,6 +42,7 @@ template <int PL_, int N_, int TWS_, int... Rs> struct SCfg {
 template <int PL_> struct RCfgT {
     static constexpr bool is_static = false;
     static constexpr bool PM_LAST = false;
+    static constexpr int GROUP_THREADS = 0;
     static constexpr int PL = PL_;
     static constexpr int SLOTS = LINE_SLOTS;
     FftDesc d; int tws_;
@@ -54,6 +56,17 @@ template <int PL_> struct RCfgT {
 // plane (a full 128-byte line per float slice) -- for kernels whose output is the float volume, at the price of 4-way bank
 // conflicts on that pass's shared-memory reads.
 template <class Base> struct PlaneMajorLast : Base { static constexpr bool PM_LAST = true; };
+
+// Grouped form: a CTA holds several independent groups of GT threads (GT = SLOTS * PL), each transforming its own line in its own
+// shared-memory buffer; the barrier between passes is the group's named barrier (1 + group index), not the CTA's.
+template <class Base, int GT> struct Grouped : Base { static constexpr int GROUP_THREADS = GT; };
+template <class Cfg> __device__ __forceinline__ int line_tid() {
+    if constexpr (Cfg::GROUP_THREADS == 0) return threadIdx.x; else return threadIdx.x % Cfg::GROUP_THREADS;
+}
+template <class Cfg> __device__ __forceinline__ void line_sync() {
+    if constexpr (Cfg::GROUP_THREADS == 0) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(1 + threadIdx.x / Cfg::GROUP_THREADS), "n"(Cfg::GROUP_THREADS) : "memory");
+}
 
 struct LineCtx {
     float2 *sm;               // [padded cell][4 planes]
@@ -101,7 +114,7 @@ __device__ __forceinline__ void line_first(const LineCtx &c, const Cfg &cfg, LD 
 #pragma unroll
         for (int k = 0; k < R; ++k) o[k * Cfg::PL] = v[k];
     }
-    __syncthreads();
+    line_sync<Cfg>();
 }
 
 // first pass when the producer already left the line in shared memory: element t = b + (n/R) j at cell R b + j
@@ -122,7 +135,7 @@ __device__ __forceinline__ void line_first_smem(const LineCtx &c, const Cfg &cfg
 #pragma unroll
         for (int k = 0; k < R; ++k) o[k * Cfg::PL] = v[k];
     }
-    __syncthreads();
+    line_sync<Cfg>();
 }
 
 // pass i (not the last): in place.  s = R1 .. R_{i-1}, ni = n / s.
@@ -157,7 +170,7 @@ __device__ __forceinline__ void line_mid(const LineCtx &c, const Cfg &cfg, int s
             for (int j = 0; j < R; ++j) c.sm[pcell(c0 + j * R1 * sub) * Cfg::PL + c.pl] = v[j];
         }
     }
-    __syncthreads();
+    line_sync<Cfg>();
 }
 
 // last pass: shared -> global (through st).  Task T = k1 + R1 (k2 + R2 (k3 + ...)) < n / R, so that the R outputs
@@ -172,7 +185,7 @@ __device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, PRE 
     const int n = cfg.n(), R1 = cfg.radix(0), ntask = n / R;
     const bool fast = (R1 & 15) == 0;
     const int step = pcell(R1) * Cfg::PL;
-    const int my_pl = Cfg::PM_LAST ? threadIdx.x / Cfg::SLOTS : c.pl, my_slot = Cfg::PM_LAST ? threadIdx.x % Cfg::SLOTS : c.slot;
+    const int my_pl = Cfg::PM_LAST ? line_tid<Cfg>() / Cfg::SLOTS : c.pl, my_slot = Cfg::PM_LAST ? line_tid<Cfg>() % Cfg::SLOTS : c.slot;
 #pragma unroll 1
     for (int T = my_slot; T < ntask; T += Cfg::SLOTS) {
         const int k1 = T % R1;
@@ -206,8 +219,9 @@ __device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, PRE 
 template <class Cfg>
 __device__ __forceinline__ LineCtx line_ctx(float2 *sm, const float2 *tw) {
     LineCtx c;
-    c.sm = sm; c.tw = tw; c.pl = threadIdx.x % Cfg::PL;
-    c.slot = threadIdx.x < Cfg::SLOTS * Cfg::PL ? threadIdx.x / Cfg::PL : (1 << 30);      // a CTA may have more threads (the gather): they only meet the barriers
+    const int tid = line_tid<Cfg>();
+    c.sm = sm; c.tw = tw; c.pl = tid % Cfg::PL;
+    c.slot = tid < Cfg::SLOTS * Cfg::PL ? tid / Cfg::PL : (1 << 30);      // a CTA may have more threads (the gather): they only meet the barriers
     return c;
 }
 

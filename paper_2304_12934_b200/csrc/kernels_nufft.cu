@@ -7,6 +7,8 @@
 // Every kernel below reads and writes whole 32-byte cells (or 16-byte halves of them).
 #include <cstdlib>
 #include <algorithm>
+#include <string>
+#include <cuda.h>          // CUtensorMap and its enums only: the encoder is fetched with cudaGetDriverEntryPoint, libcuda is not linked
 #include "common.cuh"
 #include "fft_line.cuh"
 
@@ -168,5 +170,6 @@ __global__ void TC_LB2 k_adj_rows(DevPlan d, const float2 *__restrict__ rowbuf, 
 
 #include "kernels_polar.cuh"
 #include "kernels_gather_tiles.cuh"
+#include "kernels_line_tma.cuh"
 
 }  // namespace tc

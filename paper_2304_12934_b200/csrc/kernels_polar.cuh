@@ -353,7 +353,11 @@ template <typename K> static void set_smem(K k, size_t bytes) {
 void launch_fwd_rows(const DevPlan &d, const float *vol, int S, int ng, float2 *rowbuf, cudaStream_t st) {
     TC_LINE_LAUNCH(k_fwd_rows, 2, 2, 0, d.fN, dim3(2 * d.n, ng), d, vol, S, rowbuf);
 }
+static bool launch_fwd_cols_tma(const DevPlan &d, const float2 *rowbuf, int ng, float2 *grid, cudaStream_t st);   // kernels_line_tma.cuh
+static bool env_is(const char *name, const char *value) { const char *e = std::getenv(name); return e && std::string(e) == value; }
 void launch_fwd_cols(const DevPlan &d, const float2 *rowbuf, int ng, float2 *grid, cudaStream_t st) {
+    static const bool plain = env_is("TC_COLS", "plain");
+    if (!plain && launch_fwd_cols_tma(d, rowbuf, ng, grid, st)) return;
     TC_LINE_LAUNCH(k_fwd_cols, 4, 2, 0, d.fN, dim3(d.G, ng), d, rowbuf, grid);
 }
 void launch_adj_cols(const DevPlan &d, const float2 *grid, int ng, float2 *rowbuf, cudaStream_t st) {
