@@ -138,6 +138,31 @@ __device__ __forceinline__ void line_first_smem(const LineCtx &c, const Cfg &cfg
     line_sync<Cfg>();
 }
 
+// first pass when the raw line sits in the SAME buffer in some other layout (brought in by TMA): every thread takes its R inputs
+// into registers (through ld), a barrier lets the whole line leave shared memory, then the results go to the work layout.
+// One task per thread: n / R == SLOTS.
+template <int R, bool INV, class Cfg, class LD>
+__device__ __forceinline__ void line_first_inplace(const LineCtx &c, const Cfg &cfg, LD ld) {
+    static_assert(Cfg::is_static, "compile-time pass list only");
+    constexpr int nb = Cfg::n() / R;
+    static_assert(nb == Cfg::SLOTS, "one first-pass task per thread");
+    const int b = c.slot;
+    float2 v[R];
+    if (b < nb) {
+#pragma unroll
+        for (int j = 0; j < R; ++j) v[j] = ld(b + nb * j, R % 2 == 0 ? j < R / 2 : 2 * (b + nb * j) < cfg.n());
+    }
+    line_sync<Cfg>();
+    if (b < nb) {
+        Bfly<R, INV>::run(v);
+        twiddle_mul<R, INV>(c.tw, b * cfg.tws(), v);
+        float2 *o = c.sm + pcell(R * b) * Cfg::PL + c.pl;
+#pragma unroll
+        for (int k = 0; k < R; ++k) o[k * Cfg::PL] = v[k];
+    }
+    line_sync<Cfg>();
+}
+
 // pass i (not the last): in place.  s = R1 .. R_{i-1}, ni = n / s.
 template <int R, bool INV, class Cfg>
 __device__ __forceinline__ void line_mid(const LineCtx &c, const Cfg &cfg, int s) {

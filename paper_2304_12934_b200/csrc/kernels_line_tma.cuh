@@ -127,3 +127,130 @@ static bool launch_fwd_cols_tma(const DevPlan &d, const float2 *rowbuf, int ng, 
     TC_COUNT_LAUNCH();
     return true;
 }
+
+// ------------------------------------------------------------------------------------------------------------------------------
+// Buffer-rotation pipeline for the other line kernels.  A task = one length-n transform of the 4 planes of one line (one phase of
+// the pruned split).  NGRP groups of threads work on NGRP tasks at a time, each in its own shared-memory buffer; the remaining
+// NBUF - NGRP buffers are being filled by TMA.  The raw line lands at the start of the buffer it will be transformed in
+// (line_first_inplace), so a line needs one buffer, not two.  Task q of a CTA belongs to group q % NGRP and buffer q % NBUF:
+//   j = q / NGRP, line slot m = q % NGRP + NGRP (j / 2), phase = j & 1      (both phases of a line stay with one group, in order)
+// and the group that finishes task q refills its buffer with task q + NBUF (one elected thread, after the group's barrier).
+// Tasks past the end of the CTA's lines are "issued" as a plain arrival, so that every buffer's barrier sees every phase.
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, int c3, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+
+template <int N, int NBUF> struct LpSmem {
+    static constexpr int BUF_BYTES = ((N + (N >> 4) + 1) * 32 + 127) / 128 * 128;
+    static constexpr int TOTAL = NBUF * BUF_BYTES + 128;
+};
+
+struct LpTask { int m, phase; bool valid; };
+
+// ISSUE(q, task, buffer, barrier): called by ONE thread; must arrive once on the barrier (arrive.expect_tx + copies, or plain arrive)
+// WORK(task, buffer): called by all threads of the task's group once the buffer is full; ends with the group's barrier
+template <class Cfg, int NGRP, int NBUF, class ISSUE, class WORK>
+__device__ __forceinline__ void line_pipeline(char *smem, int M, ISSUE issue, WORK work) {
+    using SM = LpSmem<Cfg::n(), NBUF>;
+    unsigned long long *full = reinterpret_cast<unsigned long long *>(smem + NBUF * SM::BUF_BYTES);
+    if (threadIdx.x == 0)
+        for (int b = 0; b < NBUF; ++b) mbar_init(&full[b], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncthreads();
+    const int J = 2 * ((M + NGRP - 1) / NGRP), Q = J * NGRP;
+    auto decode = [&](int q) { LpTask t; const int j = q / NGRP; t.m = q % NGRP + NGRP * (j >> 1); t.phase = j & 1; t.valid = t.m < M; return t; };
+    auto fill = [&](int q) {
+        const LpTask t = decode(q);
+        const int b = q % NBUF;
+        if (t.valid) issue(t, smem + b * SM::BUF_BYTES, &full[b]); else mbar_arrive(&full[b]);
+    };
+    if (threadIdx.x == 0)
+        for (int q = 0; q < NBUF && q < Q; ++q) fill(q);
+    const int gr = threadIdx.x / Cfg::GROUP_THREADS;
+    for (int j = 0; j < J; ++j) {
+        const int q = j * NGRP + gr, b = q % NBUF;
+        const LpTask t = decode(q);
+        mbar_wait(&full[b], (q / NBUF) & 1);
+        if (t.valid) work(t, smem + b * SM::BUF_BYTES);
+        if (line_tid<Cfg>() == 0 && q + NBUF < Q) { fence_proxy_async(); fill(q + NBUF); }
+    }
+}
+
+// B3 inverse row FFT + B4 (k_adj_rows, kernels_nufft.cu) on the pipeline.  Input: the adjoint half-plane rowbuf[g][x][i]; row i,
+// phase p takes x = 2 k + p, k < n: one 4-D tensor box {8 floats, 1 row i, 1 parity, 256 k} per 256 elements.
+template <class Cfg, int NGRP, int NBUF>
+__global__ void __launch_bounds__(NGRP * Cfg::GROUP_THREADS, 1) k_adj_rows_tma(DevPlan d, const __grid_constant__ CUtensorMap tm, int S, int ng,
+                                                                             float *vol) {
+    extern __shared__ __align__(128) char lt_smem[];
+    const PlaneMajorLast<Cfg> cfg{};
+    constexpr int n = Cfg::n(), R0 = Cfg::radix(0);
+    const int nlines = n * ng;
+    if ((int)blockIdx.x >= nlines) return;
+    const int M = (nlines - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int tid = line_tid<Cfg>(), pl = tid % Cfg::PL, plo = tid / Cfg::SLOTS;     // plane in the passes / in the plane-major last pass
+    line_pipeline<Cfg, NGRP, NBUF>(lt_smem, M,
+        [&](const LpTask &t, char *buf, unsigned long long *bar) {
+            const int line = blockIdx.x + t.m * gridDim.x, g = line / n, i = line - g * n;
+            mbar_arrive_expect_tx(bar, n * 32);
+#pragma unroll
+            for (int k0 = 0; k0 < n; k0 += LT_BOX_ROWS) tma_load_4d(buf + k0 * 32, &tm, 0, i, t.phase, g * n + k0, bar);
+        },
+        [&](const LpTask &t, char *buf) {
+            const int line = blockIdx.x + t.m * gridDim.x, g = line / n, i = line - g * n, p = t.phase;
+            float2 *sm = reinterpret_cast<float2 *>(buf);
+            const LineCtx c = line_ctx<PlaneMajorLast<Cfg>>(sm, d.twG);
+            const float di = d.deapod[i];
+            const int sre = 8 * g + 2 * plo;
+            const bool hre = sre < S, him = sre + 1 < S;
+            float *vre = vol + ((size_t)sre * n + i) * n, *vim = vre + (size_t)n * n;
+            line_first_inplace<R0, true>(c, cfg, [&](int k, bool) { return sm[k * 4 + pl]; });
+            static_finish<true, PlaneMajorLast<Cfg>, 1, R0>(c, cfg,
+                [&](int tt, bool lo) {                                              // this thread wrote them in phase 0
+                    const int j = wrapped(tt, n, lo).img;
+                    return p ? make_float2(hre ? vre[j] : 0.f, him ? vim[j] : 0.f) : make_float2(0.f, 0.f);
+                },
+                [&](int tt, bool lo, float2 v, float2 old) {
+                    const Wrapped w = wrapped(tt, n, lo);
+                    const float sc = di * __ldg(&d.deapod[w.img]);
+                    if (p) v = cmulc(v, __ldg(&d.twG[w.X]));
+                    v.x = fmaf(v.x, sc, old.x); v.y = fmaf(v.y, sc, old.y);
+                    if (hre) vre[w.img] = v.x;
+                    if (him) vim[w.img] = v.y;
+                });
+            line_sync<PlaneMajorLast<Cfg>>();                                      // the last pass has read the buffer
+        });
+}
+
+static int lt_sm_count() {
+    static int n_sm = 0;
+    if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
+    return n_sm;
+}
+
+// tensor-map cache of one call site: re-encoded when the buffer or the number of groups changes
+struct LtMapCache { const void *ptr = nullptr; int ng = 0, n = 0; CUtensorMap tm; };
+
+static bool launch_adj_rows_tma(const DevPlan &d, const float2 *rowbuf, int S, int ng, float *vol, cudaStream_t st) {
+    if (d.n != 2048) return false;
+    tc_encode_tiled_fn enc = tensor_map_encoder();
+    if (!enc) return false;
+    using Cfg = Grouped<SCfg<4, 2048, 2, 16, 16, 8>, 512>;
+    constexpr int NGRP = 2, NBUF = 3;
+    static LtMapCache c;
+    if (c.ptr != rowbuf || c.ng != ng || c.n != d.n) {
+        const cuuint64_t n = d.n;
+        const cuuint64_t dims[4] = {8, n, 2, n * ng};
+        const cuuint64_t strides[3] = {32, n * 32, 2 * n * 32};
+        const cuuint32_t box[4] = {8, 1, 1, LT_BOX_ROWS}, es[4] = {1, 1, 1, 1};
+        if (enc(&c.tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float2 *>(rowbuf), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { c.ptr = nullptr; return false; }
+        c.ptr = rowbuf; c.ng = ng; c.n = d.n;
+    }
+    constexpr int sh = LpSmem<2048, NBUF>::TOTAL;
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(k_adj_rows_tma<Cfg, NGRP, NBUF>, cudaFuncAttributeMaxDynamicSharedMemorySize, sh); attr = true; }
+    k_adj_rows_tma<Cfg, NGRP, NBUF><<<std::min(lt_sm_count(), d.n * ng), NGRP * Cfg::GROUP_THREADS, sh, st>>>(d, c.tm, S, ng, vol);
+    TC_COUNT_LAUNCH();
+    return true;
+}

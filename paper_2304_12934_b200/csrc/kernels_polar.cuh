@@ -363,7 +363,10 @@ void launch_fwd_cols(const DevPlan &d, const float2 *rowbuf, int ng, float2 *gri
 void launch_adj_cols(const DevPlan &d, const float2 *grid, int ng, float2 *rowbuf, cudaStream_t st) {
     TC_LINE_LAUNCH(k_adj_cols, 4, 2, 0, d.fN, dim3(d.G, ng), d, grid, rowbuf);
 }
+static bool launch_adj_rows_tma(const DevPlan &d, const float2 *rowbuf, int S, int ng, float *vol, cudaStream_t st);   // kernels_line_tma.cuh
 void launch_adj_rows(const DevPlan &d, const float2 *rowbuf, int S, int ng, float *vol, cudaStream_t st) {
+    static const bool plain = env_is("TC_AROWS", "plain");
+    if (!plain && launch_adj_rows_tma(d, rowbuf, S, ng, vol, st)) return;
     TC_LINE_LAUNCH(k_adj_rows, 4, 2, 0, d.fN, dim3(d.n, ng), d, rowbuf, S, vol);
 }
 void launch_fwd_gather(const DevPlan &d, const float2 *grid, int S, int ng, float *sino, cudaStream_t st) {
