@@ -235,7 +235,10 @@ __global__ void TC_LB k_fwd_radial(DevPlan d, const float2 *__restrict__ cpol, i
         });
 }
 
+static bool launch_fwd_radial_tma(const DevPlan &d, const float2 *cpol, int S, int ng, float *sino, cudaStream_t st);   // kernels_line_tma.cuh
 void launch_fwd_radial(const DevPlan &d, const float2 *cpol, int S, int ng, float *sino, cudaStream_t st) {
+    static const bool plain = env_is("TC_FRAD", "plain");
+    if (!plain && launch_fwd_radial_tma(d, cpol, S, ng, sino, st)) return;
     TC_LINE_LAUNCH(k_fwd_radial, 4, 1, 0, d.fD, dim3(d.na, ng), d, cpol, S, sino);
 }
 void launch_gt_keys(const DevPlan &d, unsigned long long *keys, cudaStream_t st) {

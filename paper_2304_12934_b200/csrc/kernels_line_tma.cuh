@@ -133,7 +133,7 @@ static bool launch_fwd_cols_tma(const DevPlan &d, const float2 *rowbuf, int ng, 
 // the pruned split).  NGRP groups of threads work on NGRP tasks at a time, each in its own shared-memory buffer; the remaining
 // NBUF - NGRP buffers are being filled by TMA.  The raw line lands at the start of the buffer it will be transformed in
 // (line_first_inplace), so a line needs one buffer, not two.  Task q of a CTA belongs to group q % NGRP and buffer q % NBUF:
-//   j = q / NGRP, line slot m = q % NGRP + NGRP (j / 2), phase = j & 1      (both phases of a line stay with one group, in order)
+//   j = q / NGRP, line slot m = q % NGRP + NGRP (j / NPH), phase = j % NPH   (the NPH phases of a line stay with one group, in order)
 // and the group that finishes task q refills its buffer with task q + NBUF (one elected thread, after the group's barrier).
 // Tasks past the end of the CTA's lines are "issued" as a plain arrival, so that every buffer's barrier sees every phase.
 __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, int c3, unsigned long long *bar) {
@@ -150,7 +150,7 @@ struct LpTask { int m, phase; bool valid; };
 
 // ISSUE(q, task, buffer, barrier): called by ONE thread; must arrive once on the barrier (arrive.expect_tx + copies, or plain arrive)
 // WORK(task, buffer): called by all threads of the task's group once the buffer is full; ends with the group's barrier
-template <class Cfg, int NGRP, int NBUF, class ISSUE, class WORK>
+template <class Cfg, int NGRP, int NBUF, int NPH, class ISSUE, class WORK>
 __device__ __forceinline__ void line_pipeline(char *smem, int M, ISSUE issue, WORK work) {
     using SM = LpSmem<Cfg::n(), NBUF>;
     unsigned long long *full = reinterpret_cast<unsigned long long *>(smem + NBUF * SM::BUF_BYTES);
@@ -158,8 +158,8 @@ __device__ __forceinline__ void line_pipeline(char *smem, int M, ISSUE issue, WO
         for (int b = 0; b < NBUF; ++b) mbar_init(&full[b], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
-    const int J = 2 * ((M + NGRP - 1) / NGRP), Q = J * NGRP;
-    auto decode = [&](int q) { LpTask t; const int j = q / NGRP; t.m = q % NGRP + NGRP * (j >> 1); t.phase = j & 1; t.valid = t.m < M; return t; };
+    const int J = NPH * ((M + NGRP - 1) / NGRP), Q = J * NGRP;
+    auto decode = [&](int q) { LpTask t; const int j = q / NGRP; t.m = q % NGRP + NGRP * (j / NPH); t.phase = j % NPH; t.valid = t.m < M; return t; };
     auto fill = [&](int q) {
         const LpTask t = decode(q);
         const int b = q % NBUF;
@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(NGRP * Cfg::GROUP_THREADS, 1) k_adj_rows_tma(D
     if ((int)blockIdx.x >= nlines) return;
     const int M = (nlines - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
     const int tid = line_tid<Cfg>(), pl = tid % Cfg::PL, plo = tid / Cfg::SLOTS;     // plane in the passes / in the plane-major last pass
-    line_pipeline<Cfg, NGRP, NBUF>(lt_smem, M,
+    line_pipeline<Cfg, NGRP, NBUF, 2>(lt_smem, M,
         [&](const LpTask &t, char *buf, unsigned long long *bar) {
             const int line = blockIdx.x + t.m * gridDim.x, g = line / n, i = line - g * n;
             mbar_arrive_expect_tx(bar, n * 32);
@@ -251,6 +251,209 @@ static bool launch_adj_rows_tma(const DevPlan &d, const float2 *rowbuf, int S, i
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(k_adj_rows_tma<Cfg, NGRP, NBUF>, cudaFuncAttributeMaxDynamicSharedMemorySize, sh); attr = true; }
     k_adj_rows_tma<Cfg, NGRP, NBUF><<<std::min(lt_sm_count(), d.n * ng), NGRP * Cfg::GROUP_THREADS, sh, st>>>(d, c.tm, S, ng, vol);
+    TC_COUNT_LAUNCH();
+    return true;
+}
+
+// B3 inverse column FFT (k_adj_cols) on the pipeline.  Input: column x of the fine grid, phase p = the contiguous run of cells
+// y = 2 k + p at grid[g][x][p n + k]; only the cells inside the sampled disc are brought in (one or two plain bulk copies).
+template <class Cfg, int NGRP, int NBUF>
+__global__ void __launch_bounds__(NGRP * Cfg::GROUP_THREADS, 1) k_adj_cols_tma(DevPlan d, const float2 *__restrict__ grid, int ng, float2 *rowbuf) {
+    extern __shared__ __align__(128) char lt_smem[];
+    const Cfg cfg{};
+    constexpr int n = Cfg::n(), G = 2 * n, R0 = Cfg::radix(0);
+    const int nlines = G * ng;
+    if ((int)blockIdx.x >= nlines) return;
+    const int M = (nlines - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int pl = line_tid<Cfg>() % Cfg::PL;
+    line_pipeline<Cfg, NGRP, NBUF, 2>(lt_smem, M,
+        [&](const LpTask &t, char *buf, unsigned long long *bar) {
+            const int line = blockIdx.x + t.m * gridDim.x, g = line / G, x = line - g * G, p = t.phase;
+            const int lim = disc_limit(x, G);
+            // live cells: k <= k1 (ky = 2 k + p >= 0) and k >= k2 (ky = 2 k + p - G < 0); found with disc_live itself
+            int K = (int)sqrtf((float)lim);
+            while ((K + 1) * (K + 1) <= lim) ++K;
+            while (K * K > lim) --K;
+            int k1 = (min(K, G / 2 - 1) - p) >> 1;                      // largest k with 2 k + p <= min(K, G/2 - 1); -1 if none
+            if (min(K, G / 2 - 1) - p < 0) k1 = -1;
+            int k2 = (max(G - K, G / 2) - p + 1) >> 1;                  // smallest k with 2 k + p >= max(G - K, G/2)
+            if (k2 <= k1 + 1) { k1 = n - 1; k2 = n; }                   // the two runs touch: one copy
+            const char *src = reinterpret_cast<const char *>(grid + (((size_t)g * G + x) * G + (size_t)p * n) * 4);
+            mbar_arrive_expect_tx(bar, (unsigned)((k1 + 1 + n - k2) * 32));
+            if (k1 >= 0) bulk_g2s(buf, src, (unsigned)(k1 + 1) * 32, bar);
+            if (k2 < n) bulk_g2s(buf + (size_t)k2 * 32, src + (size_t)k2 * 32, (unsigned)(n - k2) * 32, bar);
+        },
+        [&](const LpTask &t, char *buf) {
+            const int line = blockIdx.x + t.m * gridDim.x, g = line / G, x = line - g * G, p = t.phase;
+            float2 *sm = reinterpret_cast<float2 *>(buf);
+            const LineCtx c = line_ctx<Cfg>(sm, d.twG);
+            const int lim = disc_limit(x, G);
+            float2 *out = rowbuf + ((size_t)g * G + x) * n * 4 + pl;                 // adjoint half-plane, column-major: [g][x][i]
+            line_first_inplace<R0, true>(c, cfg, [&](int k, bool) { return disc_live(2 * k + p, G, lim) ? sm[k * 4 + pl] : make_float2(0.f, 0.f); });
+            static_finish<true, Cfg, 1, R0>(c, cfg,
+                [&](int tt, bool lo) { return p ? out[wrapped(tt, n, lo).img * 4] : make_float2(0.f, 0.f); },   // this thread wrote it in phase 0
+                [&](int tt, bool lo, float2 v, float2 old) {
+                    const Wrapped w = wrapped(tt, n, lo);
+                    if (p) { v = cmulc(v, __ldg(&d.twG[w.X])); v = cadd(v, old); }
+                    out[w.img * 4] = v;
+                });
+            line_sync<Cfg>();
+        });
+}
+
+// Raw layout of a line that arrives as 8 float rows (one per slice of the group): row s at float offset s (n + 4), so that the
+// four planes of a quad read four different bank groups.
+template <int N> __device__ __forceinline__ int lt_frow(int s) { return s * (N + 4); }
+
+// bulk copies of the rows of slices 8 g .. 8 g + 7 (those below S) of a [slice][line][n] float array
+template <int N>
+__device__ __forceinline__ void lt_issue_float_rows(const float *base, size_t slice_stride, size_t line_off, int g, int S, char *buf,
+                                                    unsigned long long *bar) {
+    const int ns = min(8, S - 8 * g);
+    mbar_arrive_expect_tx(bar, (unsigned)ns * N * 4);
+    for (int s = 0; s < ns; ++s)
+        bulk_g2s(buf + (size_t)lt_frow<N>(s) * 4, base + (size_t)(8 * g + s) * slice_stride + line_off, N * 4, bar);
+}
+
+// F1 + row FFT (k_fwd_rows) on the pipeline: whole 32-byte cells are stored (4-plane groups).
+template <class Cfg, int NGRP, int NBUF>
+__global__ void __launch_bounds__(NGRP * Cfg::GROUP_THREADS, 1) k_fwd_rows_tma(DevPlan d, const float *__restrict__ vol, int S, int ng,
+                                                                             float2 *__restrict__ rowbuf) {
+    extern __shared__ __align__(128) char lt_smem[];
+    const Cfg cfg{};
+    constexpr int n = Cfg::n(), G = 2 * n, R0 = Cfg::radix(0);
+    const int nlines = n * ng;
+    if ((int)blockIdx.x >= nlines) return;
+    const int M = (nlines - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int pl = line_tid<Cfg>() % Cfg::PL;
+    line_pipeline<Cfg, NGRP, NBUF, 2>(lt_smem, M,
+        [&](const LpTask &t, char *buf, unsigned long long *bar) {
+            const int line = blockIdx.x + t.m * gridDim.x, g = line / n, i = line - g * n;
+            lt_issue_float_rows<n>(vol, (size_t)n * n, (size_t)i * n, g, S, buf, bar);
+        },
+        [&](const LpTask &t, char *buf) {
+            const int line = blockIdx.x + t.m * gridDim.x, g = line / n, i = line - g * n, p = t.phase;
+            float2 *sm = reinterpret_cast<float2 *>(buf);
+            const float *rf = reinterpret_cast<const float *>(buf);
+            const LineCtx c = line_ctx<Cfg>(sm, d.twG);
+            const float di = d.deapod[i];
+            const int sre = 8 * g + 2 * pl;
+            const bool hre = sre < S, him = sre + 1 < S;
+            const float *rre = rf + lt_frow<n>(2 * pl), *rim = rf + lt_frow<n>(2 * pl + 1);
+            float2 *out = rowbuf + ((size_t)g * n + i) * G * 4 + pl;
+            line_first_inplace<R0, false>(c, cfg, [&](int tt, bool lo) {
+                const Wrapped w = wrapped(tt, n, lo);
+                const float sc = di * __ldg(&d.deapod[w.img]);
+                float2 v = make_float2(hre ? rre[w.img] * sc : 0.f, him ? rim[w.img] * sc : 0.f);
+                if (p) v = cmul(v, __ldg(&d.twG[w.X]));
+                return v;
+            });
+            static_finish<false, Cfg, 1, R0>(c, cfg, NoPre(), [&](int r, bool, float2 v, float2) { out[(size_t)(p * n + r) * 4] = v; });
+            line_sync<Cfg>();
+        });
+}
+
+// B1 radial FFT + conjugate phase (k_adj_radial) on the pipeline: one phase per line (a, g).
+template <class Cfg, int NGRP, int NBUF>
+__global__ void __launch_bounds__(NGRP * Cfg::GROUP_THREADS, 1) k_adj_radial_tma(DevPlan d, const float *__restrict__ sino, int S, int ng,
+                                                                               float2 *__restrict__ cpol) {
+    extern __shared__ __align__(128) char lt_smem[];
+    const Cfg cfg{};
+    constexpr int nd = Cfg::n(), R0 = Cfg::radix(0);
+    const int nlines = d.na * ng;
+    if ((int)blockIdx.x >= nlines) return;
+    const int M = (nlines - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int pl = line_tid<Cfg>() % Cfg::PL;
+    line_pipeline<Cfg, NGRP, NBUF, 1>(lt_smem, M,
+        [&](const LpTask &t, char *buf, unsigned long long *bar) {
+            const int line = blockIdx.x + t.m * gridDim.x, g = line / d.na, a = line - g * d.na;
+            lt_issue_float_rows<nd>(sino, (size_t)d.na * nd, (size_t)a * nd, g, S, buf, bar);
+        },
+        [&](const LpTask &t, char *buf) {
+            const int line = blockIdx.x + t.m * gridDim.x, g = line / d.na, a = line - g * d.na;
+            float2 *sm = reinterpret_cast<float2 *>(buf);
+            const float *rf = reinterpret_cast<const float *>(buf);
+            const LineCtx c = line_ctx<Cfg>(sm, d.twD);
+            const int sre = 8 * g + 2 * pl;
+            const bool hre = sre < S, him = sre + 1 < S;
+            const float *rre = rf + lt_frow<nd>(2 * pl), *rim = rf + lt_frow<nd>(2 * pl + 1);
+            float2 *out = cpol + ((size_t)g * d.na + a) * nd * 4 + pl;
+            line_first_inplace<R0, false>(c, cfg, [&](int u, bool) { return make_float2(hre ? rre[u] : 0.f, him ? rim[u] : 0.f); });
+            static_finish<false, Cfg, 1, R0>(c, cfg, NoPre(), [&](int k, bool, float2 v, float2) { out[(size_t)k * 4] = cmul(v, __ldg(&d.ph_adj[k])); });
+            line_sync<Cfg>();
+        });
+}
+
+// F4 centre phase + inverse radial FFT (k_fwd_radial) on the pipeline; plane-major last pass (whole 128-byte lines of one slice).
+template <class Cfg, int NGRP, int NBUF>
+__global__ void __launch_bounds__(NGRP * Cfg::GROUP_THREADS, 1) k_fwd_radial_tma(DevPlan d, const float2 *__restrict__ cpol, int S, int ng,
+                                                                               float *__restrict__ sino) {
+    extern __shared__ __align__(128) char lt_smem[];
+    const PlaneMajorLast<Cfg> cfg{};
+    constexpr int nd = Cfg::n(), R0 = Cfg::radix(0);
+    const int nlines = d.na * ng;
+    if ((int)blockIdx.x >= nlines) return;
+    const int M = (nlines - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int tid = line_tid<Cfg>(), pl = tid % Cfg::PL, plo = tid / Cfg::SLOTS;
+    line_pipeline<Cfg, NGRP, NBUF, 1>(lt_smem, M,
+        [&](const LpTask &t, char *buf, unsigned long long *bar) {
+            const int line = blockIdx.x + t.m * gridDim.x;
+            mbar_arrive_expect_tx(bar, nd * 32);
+            bulk_g2s(buf, cpol + (size_t)line * nd * 4, nd * 32, bar);
+        },
+        [&](const LpTask &t, char *buf) {
+            const int line = blockIdx.x + t.m * gridDim.x, g = line / d.na, a = line - g * d.na;
+            float2 *sm = reinterpret_cast<float2 *>(buf);
+            const LineCtx c = line_ctx<PlaneMajorLast<Cfg>>(sm, d.twD);
+            const int sre = 8 * g + 2 * plo;
+            const bool hre = sre < S, him = sre + 1 < S;
+            float *ore = sino + ((size_t)sre * d.na + a) * nd, *oim = ore + (size_t)d.na * nd;
+            line_first_inplace<R0, true>(c, cfg, [&](int k, bool) {
+                return 2 * k == nd ? make_float2(0.f, 0.f) : cmul(sm[k * 4 + pl], __ldg(&d.ph_fwd[k]));     // the Nyquist cell of cpol is never written
+            });
+            static_finish<true, PlaneMajorLast<Cfg>, 1, R0>(c, cfg, NoPre(), [&](int u, bool, float2 v, float2) {
+                if (hre) ore[u] = v.x;
+                if (him) oim[u] = v.y;
+            });
+            line_sync<PlaneMajorLast<Cfg>>();
+        });
+}
+
+template <class K> static void lt_set_smem(K k, int bytes) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes); }
+using LtCfgN = Grouped<SCfg<4, 2048, 2, 16, 16, 8>, 512>;       // image-side lines, n = 2048 (twiddle stride 2 in the length-G table)
+using LtCfgD = Grouped<SCfg<4, 2048, 1, 16, 16, 8>, 512>;       // radial lines, nd = 2048
+constexpr int LT_NGRP = 2, LT_NBUF = 3;
+static bool lt_aligned16(const void *q) { return (reinterpret_cast<size_t>(q) & 15) == 0; }
+
+static bool launch_adj_cols_tma(const DevPlan &d, const float2 *grid, int ng, float2 *rowbuf, cudaStream_t st) {
+    if (d.n != 2048) return false;
+    static bool attr = false;
+    if (!attr) { lt_set_smem(k_adj_cols_tma<LtCfgN, LT_NGRP, LT_NBUF>, LpSmem<2048, LT_NBUF>::TOTAL); attr = true; }
+    k_adj_cols_tma<LtCfgN, LT_NGRP, LT_NBUF><<<std::min(lt_sm_count(), d.G * ng), LT_NGRP * 512, LpSmem<2048, LT_NBUF>::TOTAL, st>>>(d, grid, ng, rowbuf);
+    TC_COUNT_LAUNCH();
+    return true;
+}
+static bool launch_fwd_rows_tma(const DevPlan &d, const float *vol, int S, int ng, float2 *rowbuf, cudaStream_t st) {
+    if (d.n != 2048 || !lt_aligned16(vol)) return false;
+    static bool attr = false;
+    if (!attr) { lt_set_smem(k_fwd_rows_tma<LtCfgN, LT_NGRP, LT_NBUF>, LpSmem<2048, LT_NBUF>::TOTAL); attr = true; }
+    k_fwd_rows_tma<LtCfgN, LT_NGRP, LT_NBUF><<<std::min(lt_sm_count(), d.n * ng), LT_NGRP * 512, LpSmem<2048, LT_NBUF>::TOTAL, st>>>(d, vol, S, ng, rowbuf);
+    TC_COUNT_LAUNCH();
+    return true;
+}
+static bool launch_adj_radial_tma(const DevPlan &d, const float *sino, int S, int ng, float2 *cpol, cudaStream_t st) {
+    if (d.nd != 2048 || !lt_aligned16(sino)) return false;
+    static bool attr = false;
+    if (!attr) { lt_set_smem(k_adj_radial_tma<LtCfgD, LT_NGRP, LT_NBUF>, LpSmem<2048, LT_NBUF>::TOTAL); attr = true; }
+    k_adj_radial_tma<LtCfgD, LT_NGRP, LT_NBUF><<<std::min(lt_sm_count(), d.na * ng), LT_NGRP * 512, LpSmem<2048, LT_NBUF>::TOTAL, st>>>(d, sino, S, ng, cpol);
+    TC_COUNT_LAUNCH();
+    return true;
+}
+static bool launch_fwd_radial_tma(const DevPlan &d, const float2 *cpol, int S, int ng, float *sino, cudaStream_t st) {
+    if (d.nd != 2048) return false;
+    static bool attr = false;
+    if (!attr) { lt_set_smem(k_fwd_radial_tma<LtCfgD, LT_NGRP, LT_NBUF>, LpSmem<2048, LT_NBUF>::TOTAL); attr = true; }
+    k_fwd_radial_tma<LtCfgD, LT_NGRP, LT_NBUF><<<std::min(lt_sm_count(), d.na * ng), LT_NGRP * 512, LpSmem<2048, LT_NBUF>::TOTAL, st>>>(d, cpol, S, ng, sino);
     TC_COUNT_LAUNCH();
     return true;
 }

@@ -350,7 +350,13 @@ template <typename K> static void set_smem(K k, size_t bytes) {
     } while (0)
 #define TC_SC(...) SCfg<__VA_ARGS__>
 
+static bool launch_fwd_rows_tma(const DevPlan &d, const float *vol, int S, int ng, float2 *rowbuf, cudaStream_t st);
+static bool launch_adj_cols_tma(const DevPlan &d, const float2 *grid, int ng, float2 *rowbuf, cudaStream_t st);
+static bool launch_adj_radial_tma(const DevPlan &d, const float *sino, int S, int ng, float2 *cpol, cudaStream_t st);
+static bool env_is(const char *name, const char *value);
 void launch_fwd_rows(const DevPlan &d, const float *vol, int S, int ng, float2 *rowbuf, cudaStream_t st) {
+    static const bool plain = env_is("TC_FROWS", "plain");
+    if (!plain && launch_fwd_rows_tma(d, vol, S, ng, rowbuf, st)) return;
     TC_LINE_LAUNCH(k_fwd_rows, 2, 2, 0, d.fN, dim3(2 * d.n, ng), d, vol, S, rowbuf);
 }
 static bool launch_fwd_cols_tma(const DevPlan &d, const float2 *rowbuf, int ng, float2 *grid, cudaStream_t st);   // kernels_line_tma.cuh
@@ -361,6 +367,8 @@ void launch_fwd_cols(const DevPlan &d, const float2 *rowbuf, int ng, float2 *gri
     TC_LINE_LAUNCH(k_fwd_cols, 4, 2, 0, d.fN, dim3(d.G, ng), d, rowbuf, grid);
 }
 void launch_adj_cols(const DevPlan &d, const float2 *grid, int ng, float2 *rowbuf, cudaStream_t st) {
+    static const bool plain = env_is("TC_ACOLS", "plain");
+    if (!plain && launch_adj_cols_tma(d, grid, ng, rowbuf, st)) return;
     TC_LINE_LAUNCH(k_adj_cols, 4, 2, 0, d.fN, dim3(d.G, ng), d, grid, rowbuf);
 }
 static bool launch_adj_rows_tma(const DevPlan &d, const float2 *rowbuf, int S, int ng, float *vol, cudaStream_t st);   // kernels_line_tma.cuh
@@ -373,6 +381,8 @@ void launch_fwd_gather(const DevPlan &d, const float2 *grid, int S, int ng, floa
     TC_LINE_LAUNCH(k_fwd_gather, 4, 1, GATHER_THREADS, d.fD, dim3(d.na, ng), d, grid, S, sino);
 }
 void launch_adj_radial(const DevPlan &d, const float *sino, int S, int ng, float2 *cpol, cudaStream_t st) {
+    static const bool plain = env_is("TC_ARAD", "plain");
+    if (!plain && launch_adj_radial_tma(d, sino, S, ng, cpol, st)) return;
     TC_LINE_LAUNCH(k_adj_radial, 4, 1, 0, d.fD, dim3(d.na, ng), d, sino, S, cpol);
 }
 void launch_spread_count(const DevPlan &d, int *counts, cudaStream_t st) {
