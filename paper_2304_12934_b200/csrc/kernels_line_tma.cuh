@@ -9,7 +9,7 @@
 //
 // k_fwd_cols_tma (F2): the two groups are the two phases of the pruned split (even / odd outputs, kernels_nufft.cu) of the SAME
 // column: they share the raw input (read from HBM once instead of once per phase) and own one work buffer each.
-//   shared memory: raw [n cells] | work 0 | work 1 | mbarriers      (n = 2048: 64 KB + 2 x 68 KB)
+//   shared memory: raw [n cells] | work 0 | work 1 | mbarriers      (n = 2048: 64 KB + 2 x 68 KB; n = 1024: two CTAs per SM)
 
 __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, unsigned long long *bar) {
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
@@ -28,7 +28,7 @@ template <int N> struct LtSmem {
 };
 
 template <class Cfg>
-__global__ void __launch_bounds__(2 * Cfg::GROUP_THREADS, 1) k_fwd_cols_tma(DevPlan d, const __grid_constant__ CUtensorMap tm, int ng,
+__global__ void __launch_bounds__(2 * Cfg::GROUP_THREADS, 1024 / (2 * Cfg::GROUP_THREADS)) k_fwd_cols_tma(DevPlan d, const __grid_constant__ CUtensorMap tm, int ng,
                                                                           float2 *__restrict__ grid) {
     extern __shared__ __align__(128) char lt_smem[];
     using SM = LtSmem<Cfg::n()>;
@@ -100,32 +100,49 @@ static int lt_l2_promotion() {
     return v;
 }
 
+// Pass list, group size and pipeline shape per line length (the lengths of BASELINE configs 3 and 4; others take the plain kernels)
+template <int N, int TWS> struct LtSize;
+template <int TWS> struct LtSize<2048, TWS> { using Cfg = Grouped<SCfg<4, 2048, TWS, 16, 16, 8>, 512>; static constexpr int NGRP = 2, NBUF = 3, CTAS = 1; };
+template <int TWS> struct LtSize<1024, TWS> { using Cfg = Grouped<SCfg<4, 1024, TWS, 16, 16, 4>, 256>; static constexpr int NGRP = 4, NBUF = 6, CTAS = 2; };
+static int lt_sm_count() {
+    static int n_sm = 0;
+    if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
+    return n_sm;
+}
+// tensor-map cache of one call site: re-encoded when the buffer or the number of groups changes
+struct LtMapCache { const void *ptr = nullptr; int ng = 0, n = 0; CUtensorMap tm; };
+
 // true if the TMA-fed kernel took the launch
-static bool launch_fwd_cols_tma(const DevPlan &d, const float2 *rowbuf, int ng, float2 *grid, cudaStream_t st) {
-    if (d.n != 2048) return false;
+template <int N>
+static bool launch_fwd_cols_tma_n(const DevPlan &d, const float2 *rowbuf, int ng, float2 *grid, cudaStream_t st) {
     tc_encode_tiled_fn enc = tensor_map_encoder();
     if (!enc) return false;
-    using Cfg = Grouped<SCfg<4, 2048, 2, 16, 16, 8>, 512>;
-    static const float2 *c_ptr = nullptr; static int c_ng = 0; static CUtensorMap c_tm;
-    if (c_ptr != rowbuf || c_ng != ng) {
+    using Cfg = typename LtSize<N, 2>::Cfg;
+    static LtMapCache c;
+    if (c.ptr != rowbuf || c.ng != ng) {
         const cuuint64_t dims[3] = {8, (cuuint64_t)d.G, (cuuint64_t)d.n * ng};
         const cuuint64_t strides[2] = {32, (cuuint64_t)d.G * 32};
         const cuuint32_t box[3] = {8, 1, LT_BOX_ROWS}, es[3] = {1, 1, 1};
         const int l2 = lt_l2_promotion();
         const CUtensorMapL2promotion pr = l2 == 1 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : l2 == 2 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
                                         : l2 == 3 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_NONE;
-        if (enc(&c_tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float2 *>(rowbuf), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                CU_TENSOR_MAP_SWIZZLE_NONE, pr, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { c_ptr = nullptr; return false; }
-        c_ptr = rowbuf; c_ng = ng;
+        if (enc(&c.tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float2 *>(rowbuf), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, pr, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { c.ptr = nullptr; return false; }
+        c.ptr = rowbuf; c.ng = ng;
     }
-    static int n_sm = 0;
-    if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
-    constexpr int sh = LtSmem<2048>::TOTAL;
+    constexpr int sh = LtSmem<N>::TOTAL;
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(k_fwd_cols_tma<Cfg>, cudaFuncAttributeMaxDynamicSharedMemorySize, sh); attr = true; }
-    k_fwd_cols_tma<Cfg><<<std::min(n_sm, d.G * ng), 2 * Cfg::GROUP_THREADS, sh, st>>>(d, c_tm, ng, grid);
+    k_fwd_cols_tma<Cfg><<<std::min(LtSize<N, 2>::CTAS * lt_sm_count(), d.G * ng), 2 * Cfg::GROUP_THREADS, sh, st>>>(d, c.tm, ng, grid);
     TC_COUNT_LAUNCH();
     return true;
+}
+static bool launch_fwd_cols_tma(const DevPlan &d, const float2 *rowbuf, int ng, float2 *grid, cudaStream_t st) {
+    switch (d.n) {
+    case 2048: return launch_fwd_cols_tma_n<2048>(d, rowbuf, ng, grid, st);
+    case 1024: return launch_fwd_cols_tma_n<1024>(d, rowbuf, ng, grid, st);
+    default: return false;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------------------------------
@@ -222,37 +239,34 @@ __global__ void __launch_bounds__(NGRP * Cfg::GROUP_THREADS, 1) k_adj_rows_tma(D
         });
 }
 
-static int lt_sm_count() {
-    static int n_sm = 0;
-    if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
-    return n_sm;
-}
-
-// tensor-map cache of one call site: re-encoded when the buffer or the number of groups changes
-struct LtMapCache { const void *ptr = nullptr; int ng = 0, n = 0; CUtensorMap tm; };
-
-static bool launch_adj_rows_tma(const DevPlan &d, const float2 *rowbuf, int S, int ng, float *vol, cudaStream_t st) {
-    if (d.n != 2048) return false;
+template <int N>
+static bool launch_adj_rows_tma_n(const DevPlan &d, const float2 *rowbuf, int S, int ng, float *vol, cudaStream_t st) {
     tc_encode_tiled_fn enc = tensor_map_encoder();
     if (!enc) return false;
-    using Cfg = Grouped<SCfg<4, 2048, 2, 16, 16, 8>, 512>;
-    constexpr int NGRP = 2, NBUF = 3;
+    using L = LtSize<N, 2>;
     static LtMapCache c;
-    if (c.ptr != rowbuf || c.ng != ng || c.n != d.n) {
+    if (c.ptr != rowbuf || c.ng != ng) {
         const cuuint64_t n = d.n;
         const cuuint64_t dims[4] = {8, n, 2, n * ng};
         const cuuint64_t strides[3] = {32, n * 32, 2 * n * 32};
         const cuuint32_t box[4] = {8, 1, 1, LT_BOX_ROWS}, es[4] = {1, 1, 1, 1};
         if (enc(&c.tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float2 *>(rowbuf), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                 CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { c.ptr = nullptr; return false; }
-        c.ptr = rowbuf; c.ng = ng; c.n = d.n;
+        c.ptr = rowbuf; c.ng = ng;
     }
-    constexpr int sh = LpSmem<2048, NBUF>::TOTAL;
+    constexpr int sh = LpSmem<N, L::NBUF>::TOTAL;
     static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(k_adj_rows_tma<Cfg, NGRP, NBUF>, cudaFuncAttributeMaxDynamicSharedMemorySize, sh); attr = true; }
-    k_adj_rows_tma<Cfg, NGRP, NBUF><<<std::min(lt_sm_count(), d.n * ng), NGRP * Cfg::GROUP_THREADS, sh, st>>>(d, c.tm, S, ng, vol);
+    if (!attr) { cudaFuncSetAttribute(k_adj_rows_tma<typename L::Cfg, L::NGRP, L::NBUF>, cudaFuncAttributeMaxDynamicSharedMemorySize, sh); attr = true; }
+    k_adj_rows_tma<typename L::Cfg, L::NGRP, L::NBUF><<<std::min(lt_sm_count(), d.n * ng), L::NGRP * L::Cfg::GROUP_THREADS, sh, st>>>(d, c.tm, S, ng, vol);
     TC_COUNT_LAUNCH();
     return true;
+}
+static bool launch_adj_rows_tma(const DevPlan &d, const float2 *rowbuf, int S, int ng, float *vol, cudaStream_t st) {
+    switch (d.n) {
+    case 2048: return launch_adj_rows_tma_n<2048>(d, rowbuf, S, ng, vol, st);
+    case 1024: return launch_adj_rows_tma_n<1024>(d, rowbuf, S, ng, vol, st);
+    default: return false;
+    }
 }
 
 // B3 inverse column FFT (k_adj_cols) on the pipeline.  Input: column x of the fine grid, phase p = the contiguous run of cells
@@ -419,41 +433,46 @@ __global__ void __launch_bounds__(NGRP * Cfg::GROUP_THREADS, 1) k_fwd_radial_tma
         });
 }
 
-template <class K> static void lt_set_smem(K k, int bytes) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes); }
-using LtCfgN = Grouped<SCfg<4, 2048, 2, 16, 16, 8>, 512>;       // image-side lines, n = 2048 (twiddle stride 2 in the length-G table)
-using LtCfgD = Grouped<SCfg<4, 2048, 1, 16, 16, 8>, 512>;       // radial lines, nd = 2048
-constexpr int LT_NGRP = 2, LT_NBUF = 3;
 static bool lt_aligned16(const void *q) { return (reinterpret_cast<size_t>(q) & 15) == 0; }
 
+// launch of a pipeline kernel KERNEL<Cfg, NGRP, NBUF> for line length N (twiddle stride TWS), `lines` lines
+#define TC_LP_LAUNCH(KERNEL, N, TWS, lines, ...)                                                                              \
+    do {                                                                                                                      \
+        using L = LtSize<N, TWS>;                                                                                             \
+        constexpr int sh = LpSmem<N, L::NBUF>::TOTAL;                                                                         \
+        static bool attr = false;                                                                                             \
+        if (!attr) { cudaFuncSetAttribute(KERNEL<typename L::Cfg, L::NGRP, L::NBUF>, cudaFuncAttributeMaxDynamicSharedMemorySize, sh); attr = true; } \
+        KERNEL<typename L::Cfg, L::NGRP, L::NBUF><<<std::min(lt_sm_count(), (lines)), L::NGRP * L::Cfg::GROUP_THREADS, sh, st>>>(__VA_ARGS__);        \
+        TC_COUNT_LAUNCH();                                                                                                    \
+    } while (0)
+
 static bool launch_adj_cols_tma(const DevPlan &d, const float2 *grid, int ng, float2 *rowbuf, cudaStream_t st) {
-    if (d.n != 2048) return false;
-    static bool attr = false;
-    if (!attr) { lt_set_smem(k_adj_cols_tma<LtCfgN, LT_NGRP, LT_NBUF>, LpSmem<2048, LT_NBUF>::TOTAL); attr = true; }
-    k_adj_cols_tma<LtCfgN, LT_NGRP, LT_NBUF><<<std::min(lt_sm_count(), d.G * ng), LT_NGRP * 512, LpSmem<2048, LT_NBUF>::TOTAL, st>>>(d, grid, ng, rowbuf);
-    TC_COUNT_LAUNCH();
-    return true;
+    switch (d.n) {
+    case 2048: TC_LP_LAUNCH(k_adj_cols_tma, 2048, 2, d.G * ng, d, grid, ng, rowbuf); return true;
+    case 1024: TC_LP_LAUNCH(k_adj_cols_tma, 1024, 2, d.G * ng, d, grid, ng, rowbuf); return true;
+    default: return false;
+    }
 }
 static bool launch_fwd_rows_tma(const DevPlan &d, const float *vol, int S, int ng, float2 *rowbuf, cudaStream_t st) {
-    if (d.n != 2048 || !lt_aligned16(vol)) return false;
-    static bool attr = false;
-    if (!attr) { lt_set_smem(k_fwd_rows_tma<LtCfgN, LT_NGRP, LT_NBUF>, LpSmem<2048, LT_NBUF>::TOTAL); attr = true; }
-    k_fwd_rows_tma<LtCfgN, LT_NGRP, LT_NBUF><<<std::min(lt_sm_count(), d.n * ng), LT_NGRP * 512, LpSmem<2048, LT_NBUF>::TOTAL, st>>>(d, vol, S, ng, rowbuf);
-    TC_COUNT_LAUNCH();
-    return true;
+    if (!lt_aligned16(vol)) return false;
+    switch (d.n) {
+    case 2048: TC_LP_LAUNCH(k_fwd_rows_tma, 2048, 2, d.n * ng, d, vol, S, ng, rowbuf); return true;
+    case 1024: TC_LP_LAUNCH(k_fwd_rows_tma, 1024, 2, d.n * ng, d, vol, S, ng, rowbuf); return true;
+    default: return false;
+    }
 }
 static bool launch_adj_radial_tma(const DevPlan &d, const float *sino, int S, int ng, float2 *cpol, cudaStream_t st) {
-    if (d.nd != 2048 || !lt_aligned16(sino)) return false;
-    static bool attr = false;
-    if (!attr) { lt_set_smem(k_adj_radial_tma<LtCfgD, LT_NGRP, LT_NBUF>, LpSmem<2048, LT_NBUF>::TOTAL); attr = true; }
-    k_adj_radial_tma<LtCfgD, LT_NGRP, LT_NBUF><<<std::min(lt_sm_count(), d.na * ng), LT_NGRP * 512, LpSmem<2048, LT_NBUF>::TOTAL, st>>>(d, sino, S, ng, cpol);
-    TC_COUNT_LAUNCH();
-    return true;
+    if (!lt_aligned16(sino)) return false;
+    switch (d.nd) {
+    case 2048: TC_LP_LAUNCH(k_adj_radial_tma, 2048, 1, d.na * ng, d, sino, S, ng, cpol); return true;
+    case 1024: TC_LP_LAUNCH(k_adj_radial_tma, 1024, 1, d.na * ng, d, sino, S, ng, cpol); return true;
+    default: return false;
+    }
 }
 static bool launch_fwd_radial_tma(const DevPlan &d, const float2 *cpol, int S, int ng, float *sino, cudaStream_t st) {
-    if (d.nd != 2048) return false;
-    static bool attr = false;
-    if (!attr) { lt_set_smem(k_fwd_radial_tma<LtCfgD, LT_NGRP, LT_NBUF>, LpSmem<2048, LT_NBUF>::TOTAL); attr = true; }
-    k_fwd_radial_tma<LtCfgD, LT_NGRP, LT_NBUF><<<std::min(lt_sm_count(), d.na * ng), LT_NGRP * 512, LpSmem<2048, LT_NBUF>::TOTAL, st>>>(d, cpol, S, ng, sino);
-    TC_COUNT_LAUNCH();
-    return true;
+    switch (d.nd) {
+    case 2048: TC_LP_LAUNCH(k_fwd_radial_tma, 2048, 1, d.na * ng, d, cpol, S, ng, sino); return true;
+    case 1024: TC_LP_LAUNCH(k_fwd_radial_tma, 1024, 1, d.na * ng, d, cpol, S, ng, sino); return true;
+    default: return false;
+    }
 }
