@@ -63,6 +63,8 @@ __host__ __device__ inline int gt_nty(int G) { return (G + 8 + GT_BY - 1) / GT_B
 
 // Window polynomial coefficients (monomial in z, c[0] + c[1] z + ...), set by the plan.
 void set_kb_coeffs(const float *h);
+// Roots of unity of the odd FFT radices (constant memory), set by the plan.
+void set_fft_roots();
 
 // ---- launch wrappers (kernels_nufft.cu).  All buffers are device memory. -------------------------
 // vol [S][n][n] -> rowbuf [ng][n][G][P] c64      (F1 pad + deapodise, row FFT)

@@ -9,7 +9,7 @@ namespace tc {
 
 constexpr int FFT_MAX_PASSES = 5;
 
-// n = radix[0] * ... * radix[npass-1]; radix-16 passes first, a radix-5 pass (if any) last; npass >= 2.
+// n = radix[0] * ... * radix[npass-1]; radix-16 passes first, then the rest of the power of two, then the odd factors (3, 7, 17, 5); npass >= 2.
 struct FftDesc {
     int n;
     int npass;
@@ -45,7 +45,34 @@ template <bool INV> __device__ __forceinline__ void bfly4(float2 &a, float2 &b, 
     b = cadd(t1, t3); d = csub(t1, t3);
 }
 
-template <int R, bool INV> struct Bfly;
+// Odd radices without a hand-written butterfly (3, 7, ...: detector sizes such as 2448 = 2^4 3^2 17): the plain DFT,
+// R (R - 1) complex multiply-adds with the roots of unity from constant memory (immediate operands after unrolling).
+constexpr int FFT_MAX_ODD = 17;
+#ifdef TC_FFT_ROOTS_DEFINE
+__constant__ float2 c_root[FFT_MAX_ODD + 1][FFT_MAX_ODD + 1];          // c_root[R][m] = e^{-2 pi i m / R}, odd R only (set_fft_roots)
+#endif
+template <int R, bool INV> struct Bfly {
+#ifdef TC_FFT_ROOTS_DEFINE
+    static_assert((R & 1) == 1 && R <= FFT_MAX_ODD, "generic butterfly: odd radices only");
+    __device__ static __forceinline__ void run(float2 (&v)[R]) {
+        float2 o[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) {
+            float2 acc = v[0];
+#pragma unroll
+            for (int j = 1; j < R; ++j) {
+                const float2 w = c_root[R][(j * k) % R];
+                const float wy = INV ? -w.y : w.y;
+                acc.x = fmaf(v[j].x, w.x, fmaf(-v[j].y, wy, acc.x));
+                acc.y = fmaf(v[j].x, wy, fmaf(v[j].y, w.x, acc.y));
+            }
+            o[k] = acc;
+        }
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k] = o[k];
+    }
+#endif
+};
 
 template <bool INV> struct Bfly<2, INV> {
     __device__ static __forceinline__ void run(float2 (&v)[2]) {

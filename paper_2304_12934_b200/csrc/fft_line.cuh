@@ -76,7 +76,16 @@ struct LineCtx {
 
 // v[k] *= w^k, w = tw[base * tws] (conjugated for the inverse); powers from tw[base], tw[2 base], tw[4 base], tw[8 base]
 template <int R, bool INV>
-__device__ __forceinline__ void twiddle_mul(const float2 *__restrict__ t, int e, float2 (&v)[R]) {
+__device__ __forceinline__ void twiddle_mul(const float2 *__restrict__ t, int e, float2 (&v)[R], int len = 0) {
+    if constexpr ((R & 1) == 1) {                      // odd radix: one table entry per factor, exponent reduced modulo the table length
+#pragma unroll
+        for (int k = 1; k < R; ++k) {
+            float2 w = __ldg(t + (k * e) % len);
+            if (INV) w.y = -w.y;
+            v[k] = cmul(v[k], w);
+        }
+        return;
+    }
     float2 w1 = __ldg(t + e);
     if (INV) w1.y = -w1.y;
     v[1] = cmul(v[1], w1);
@@ -186,7 +195,7 @@ __device__ __forceinline__ void line_mid(const LineCtx &c, const Cfg &cfg, int s
             for (int j = 0; j < R; ++j) v[j] = c.sm[pcell(c0 + j * R1 * sub) * Cfg::PL + c.pl];
         }
         Bfly<R, INV>::run(v);
-        twiddle_mul<R, INV>(c.tw, bi * s * cfg.tws(), v);
+        twiddle_mul<R, INV>(c.tw, bi * s * cfg.tws(), v, n * cfg.tws());
         if (fast) {
 #pragma unroll
             for (int j = 0; j < R; ++j) p0[j * step] = v[j];
@@ -272,7 +281,11 @@ __device__ __forceinline__ void runtime_finish(const LineCtx &c, const Cfg &cfg,
         if (R == 16) line_mid<16, INV>(c, cfg, s);
         else if (R == 8) line_mid<8, INV>(c, cfg, s);
         else if (R == 4) line_mid<4, INV>(c, cfg, s);
-        else line_mid<2, INV>(c, cfg, s);
+        else if (R == 2) line_mid<2, INV>(c, cfg, s);
+        else if (R == 3) line_mid<3, INV>(c, cfg, s);
+        else if (R == 5) line_mid<5, INV>(c, cfg, s);
+        else if (R == 7) line_mid<7, INV>(c, cfg, s);
+        else line_mid<17, INV>(c, cfg, s);
         s *= R;
     }
     const int RL = cfg.radix(cfg.npass() - 1);
@@ -280,7 +293,10 @@ __device__ __forceinline__ void runtime_finish(const LineCtx &c, const Cfg &cfg,
     else if (RL == 8) line_last<8, INV>(c, cfg, pre, st);
     else if (RL == 5) line_last<5, INV>(c, cfg, pre, st);
     else if (RL == 4) line_last<4, INV>(c, cfg, pre, st);
-    else line_last<2, INV>(c, cfg, pre, st);
+    else if (RL == 2) line_last<2, INV>(c, cfg, pre, st);
+    else if (RL == 3) line_last<3, INV>(c, cfg, pre, st);
+    else if (RL == 7) line_last<7, INV>(c, cfg, pre, st);
+    else line_last<17, INV>(c, cfg, pre, st);
 }
 
 // global -> FFT -> global.  ld(t, lo) returns this thread's plane of input element t; st(k, lo, v, old) takes output k.

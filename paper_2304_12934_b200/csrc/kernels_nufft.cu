@@ -9,6 +9,7 @@
 #include <algorithm>
 #include <string>
 #include <cuda.h>          // CUtensorMap and its enums only: the encoder is fetched with cudaGetDriverEntryPoint, libcuda is not linked
+#define TC_FFT_ROOTS_DEFINE       // this translation unit owns the constant table of the odd butterflies
 #include "common.cuh"
 #include "fft_line.cuh"
 
@@ -16,6 +17,15 @@ namespace tc {
 
 __constant__ float c_kb[KB_DEG + 1];
 void set_kb_coeffs(const float *h) { cudaMemcpyToSymbol(c_kb, h, sizeof(float) * (KB_DEG + 1)); }
+void set_fft_roots() {
+    static float2 h[FFT_MAX_ODD + 1][FFT_MAX_ODD + 1];
+    for (int R = 1; R <= FFT_MAX_ODD; ++R)
+        for (int m = 0; m <= FFT_MAX_ODD; ++m) {
+            const double a = 2.0 * 3.14159265358979323846 * (m % R) / R;
+            h[R][m] = make_float2((float)cos(a), (float)-sin(a));
+        }
+    cudaMemcpyToSymbol(c_root, h, sizeof(h));
+}
 
 long long &launch_counter() { static thread_local long long c = 0; return c; }
 

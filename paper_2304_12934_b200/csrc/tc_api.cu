@@ -126,18 +126,20 @@ static void kb_poly(int W, double sigma, float *out) {
     }
 }
 
-// n = 2^a 5^b (b <= 1) as a pass list for the line engine: radix-16 passes first, then 8 / 4 / 2, the radix-5 pass last.
+// n = 2^a 3^b 5^c 7^d 17^e (a >= 1) as a pass list for the line engine: radix-16 passes first, then 8 / 4 / 2, then the odd
+// factors 3, 7, 17 and 5 (one pass each; 5 last, as the compile-time list of n = 2560 has it); at most FFT_MAX_PASSES passes.
 static bool make_fft_desc(int n, FftDesc &f) {
-    int m = n, fives = 0, twos = 0;
-    while (m % 5 == 0) { m /= 5; ++fives; }
+    int m = n, twos = 0, odd[4] = {0, 0, 0, 0};
+    const int primes[4] = {3, 7, 17, 5};
     while (m % 2 == 0) { m /= 2; ++twos; }
-    if (m != 1 || fives > 1) return false;
+    for (int q = 0; q < 4; ++q) while (m % primes[q] == 0) { m /= primes[q]; ++odd[q]; }
+    if (m != 1 || twos < 1) return false;
     f.n = n; f.npass = 0;
-    while (twos >= 4) { f.radix[f.npass++] = 16; twos -= 4; if (f.npass >= FFT_MAX_PASSES - 1) break; }
-    if (twos >= 4) return false;
-    if (twos > 0) f.radix[f.npass++] = 1 << twos;
-    if (fives) f.radix[f.npass++] = 5;
-    if (f.npass < 2) {                              // 16 -> 4 x 4, 8 -> 4 x 2, 4 -> 2 x 2; 2 and 5 alone are not supported
+    auto push = [&](int r) { if (f.npass >= FFT_MAX_PASSES) return false; f.radix[f.npass++] = r; return true; };
+    while (twos >= 4) { if (!push(16)) return false; twos -= 4; }
+    if (twos > 0 && !push(1 << twos)) return false;
+    for (int q = 0; q < 4; ++q) for (int k = 0; k < odd[q]; ++k) if (!push(primes[q])) return false;
+    if (f.npass < 2) {                              // 16 -> 4 x 4, 8 -> 4 x 2, 4 -> 2 x 2; 2 alone is not supported
         if (f.npass == 1 && f.radix[0] >= 4) { const int r = f.radix[0]; f.radix[0] = r == 4 ? 2 : 4; f.radix[1] = r / f.radix[0]; f.npass = 2; }
         else return false;
     }
@@ -168,7 +170,7 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
     const int n = gm->n, nd = gm->n_det, na = gm->n_angles, G = 2 * n;
     DevPlan &d = p->d;
     d.n = n; d.nd = nd; d.na = na; d.G = G; d.sc = (double)G / nd;
-    if (!make_fft_desc(n, d.fN) || !make_fft_desc(nd, d.fD)) { delete p; return fail(TC_EUNSUPPORTED, "n and n_det must be 2^a 5^b with b <= 1 (and at most 6800)"); }
+    if (!make_fft_desc(n, d.fN) || !make_fft_desc(nd, d.fD)) { delete p; return fail(TC_EUNSUPPORTED, "n and n_det must be 2^a 3^b 5^c 7^d 17^e, a >= 1, with at most 5 FFT passes (and at most 6800)"); }
     if (nd / 2 - 1 > 0 && d.sc * (nd / 2 - 1) + 3 >= G / 2 + 3) { /* taps wrap at most once; always true for sc = G/nd */ }
 
     const int W = KB_W; const double sigma = 2.0;
@@ -176,6 +178,7 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
     float kb[KB_DEG + 1];
     kb_poly(W, sigma, kb);
     set_kb_coeffs(kb);
+    set_fft_roots();
     std::vector<float> deapod(n);
     for (int j = 0; j < n; ++j) {
         const double x = j - n / 2, a = M_PI * W * x / G, s = std::sqrt(beta * beta - a * a);

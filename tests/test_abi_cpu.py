@@ -28,7 +28,7 @@ def test_argument_validation_without_gpu():
     ang = np.zeros(4, dtype=np.float32)
     for kw, status in ((dict(n=63, n_det=64), tc.TC_EINVAL), (dict(n=64, n_det=63), tc.TC_EINVAL),
                        (dict(n=0, n_det=64), tc.TC_EINVAL), (dict(n=48, n_det=64), tc.TC_EUNSUPPORTED),
-                       (dict(n=96, n_det=96), tc.TC_EUNSUPPORTED)):
+                       (dict(n=352, n_det=64), tc.TC_EUNSUPPORTED), (dict(n=64, n_det=26), tc.TC_EUNSUPPORTED)):      # factors 11, 13
         with pytest.raises(tc.TcError) as e:
             tc.Plan(kw["n"], kw["n_det"], ang)
         assert e.value.status == status, kw

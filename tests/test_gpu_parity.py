@@ -83,6 +83,12 @@ def test_config2_forward_adjoint(tc):
     (2, 128, 256, 20, 130.0),    # n_det = 2 n  (one fine-grid cell per radial mode)
     (2, 128, 64, 20, 30.0),      # n_det = n / 2 (four cells per mode)
     (17, 32, 32, 5, 16.0),       # smallest supported image, three groups
+    (2, 64, 48, 9, 25.5),        # odd radices: n_det = 2^4 3
+    (3, 96, 144, 11, 70.0),      # n = 2^5 3 (G = 192 = 16 4 3), n_det = 2^4 3^2 (radix-3 mid pass and last pass)
+    (2, 64, 272, 6, 140.25),     # n_det = 2^4 17
+    (2, 224, 112, 8, 57.0),      # n = 2^5 7, n_det = 2^4 7
+    (2, 160, 200, 7, 99.0),      # n_det = 2^3 5^2 (two radix-5 passes)
+    (9, 128, 306, 10, 150.5),    # n_det = 2 3^2 17: the factors of the paper's 2448-bin detector (radix 2, 3, 3, 17)
 ])
 def test_shapes_and_ragged_tails(tc, S, N, Nd, Na, centre):
     from oracle import nufft
@@ -350,6 +356,27 @@ def test_full_size_config3_and_config5_geometry_sampled(tc):
         plan.close()
         assert rel_l2(b[3], nufft.backproject_nufft(y[3], a64, c["N"], c["centre"])) < TOL_NUFFT
         assert _adj_mismatch(vol, y, s, b) < TOL_ADJ
+
+
+def test_second_workload_shape_2448_bins(tc):
+    # the shape of the paper's third data set (202 projections x 2448 columns, Table 1) on a 2560^2 image:
+    # n_det = 2448 = 2^4 3^2 17 runs the radix-3 and radix-17 passes of the radial FFT, n_det != n puts 2.09 fine-grid cells between
+    # radial modes.  8 slices; one slice against the oracle NUFFT, two angles against the direct DFT, adjoint identity.
+    from paper_2304_12934_b200 import inputs
+    from oracle import nufft, direct
+    N, Nd, Na, centre = 2560, 2448, 202, 1221.75
+    ang = inputs.angles_uniform(Na); a64 = ang.astype(np.float64)
+    vol = inputs.volume_fibres(8, N, 1086, n_fibres=400)
+    plan = tc.Plan(N, Nd, ang, centre)
+    s = _np(plan.radon(_cuda(vol)))
+    assert rel_l2(s[5], nufft.radon_nufft(vol[5], a64, Nd, centre)) < TOL_NUFFT
+    sel = [17, 160]
+    assert rel_l2(s[5][sel], direct.radon_direct(vol[5], a64[sel], Nd, centre)) < TOL_DIRECT
+    y = np.random.default_rng(86).standard_normal(s.shape).astype(np.float32)
+    b = _np(plan.backproject(_cuda(y)))
+    plan.close()
+    assert rel_l2(b[2], nufft.backproject_nufft(y[2], a64, N, centre)) < TOL_NUFFT
+    assert _adj_mismatch(vol, y, s, b) < TOL_ADJ
 
 
 def test_fbp_vs_oracle(tc):
