@@ -80,10 +80,13 @@ tc_status tc_backproject(tc_plan *plan, const float *sinogram, int n_slices, flo
 
 /* Filtered back-projection, eq. (4) P:L64 (f = R* F^-1 |k| F p; filters P:L68): tc_backproject with every radial mode m weighted
  * by (pi / n_angles) * r(m) * win(m), r = |m| / n_det (1 / (4 n_det) at m = 0, the mean of |k| over the DC bin), win = 1 for
- * TC_FILTER_RAMP or 0.5 (1 + cos(2 pi m / n_det)) for TC_FILTER_HANN, so that tc_fbp(tc_radon(f)) ~ f for angles uniform in [0, pi).
+ * TC_FILTER_RAMP, 0.5 (1 + cos(2 pi m / n_det)) for TC_FILTER_HANN, and the Shepp-Logan and Butterworth windows below (the filters
+ * P:L68 names), so that tc_fbp(tc_radon(f)) ~ f for angles uniform in [0, pi).
  * Same pointers, layouts, slab streaming and stream semantics as tc_backproject.  TC_EINVAL for an unknown filter. */
-#define TC_FILTER_RAMP 0
+#define TC_FILTER_RAMP 0          /* Ram-Lak */
 #define TC_FILTER_HANN 1
+#define TC_FILTER_SHEPP_LOGAN 2   /* ramp x sin(pi m / n_det) / (pi m / n_det) */
+#define TC_FILTER_BUTTERWORTH 3   /* ramp / (1 + (|m| / (n_det / 4))^4): order 2, cut-off at half the Nyquist frequency */
 tc_status tc_fbp(tc_plan *plan, const float *sinogram, int n_slices, int filter, float *volume, void *cuda_stream);
 
 /* Pre-pass for measured data ("b = -log(I / I0)", P:L129 sinogram order): Beer-Lambert transform and the reorder from

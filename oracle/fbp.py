@@ -6,8 +6,10 @@ radial mode m weighted by
 
     rho[m] = (pi / Na) * r(|m| / Nd) * win(m),     r(k) = k for m != 0,   r = 1 / (4 Nd) at m = 0
 
-(the mean of |k| over the DC bin [-1/(2 Nd), 1/(2 Nd)], so the reconstruction keeps its mean), win = 1 (ramp) or the Hann
-window 0.5 (1 + cos(2 pi m / Nd)).  The Nyquist mode is excluded like everywhere else (G2).
+(the mean of |k| over the DC bin [-1/(2 Nd), 1/(2 Nd)], so the reconstruction keeps its mean), win = 1 (ramp = Ram-Lak), the Hann
+window 0.5 (1 + cos(2 pi m / Nd)), Shepp-Logan sinc(m / Nd) = sin(pi m / Nd) / (pi m / Nd), or Butterworth 1 / (1 + (x / 0.5)^4),
+x = |m| / (Nd / 2) (order 2, cut-off at half the Nyquist frequency); the filters the paper names.
+The Nyquist mode is excluded like everywhere else (G2).
 
   fbp_direct   the definition, O(Na Nd N^2)
   fbp_nufft    the same weights inside the oracle's NUFFT adjoint (radial_forward -> weight -> spread -> ifft2 -> crop)
@@ -27,6 +29,10 @@ def ramp_weights(nd, na, window="ramp"):
     r[m == 0] = 0.25 / nd
     if window == "hann":
         r = r * 0.5 * (1.0 + np.cos(2.0 * np.pi * m / nd))
+    elif window == "shepp-logan":
+        r = r * np.sinc(m / nd)                                     # numpy's sinc(x) = sin(pi x) / (pi x)
+    elif window == "butterworth":
+        r = r / (1.0 + (np.abs(m) / (nd / 2.0) / 0.5) ** 4)
     elif window != "ramp":
         raise ValueError(window)
     return (np.pi / na) * r

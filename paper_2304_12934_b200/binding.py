@@ -147,7 +147,7 @@ class Plan:
         S = sinogram.shape[0]
         assert tuple(sinogram.shape) == (S, self.n_angles, self.n_det)
         out = _like(sinogram, (S, self.n, self.n)) if out is None else out
-        _check(lib.tc_fbp(self._h, _ptr(sinogram), S, {"ramp": 0, "hann": 1}[filter], _ptr(out), _stream(sinogram)))
+        _check(lib.tc_fbp(self._h, _ptr(sinogram), S, {"ramp": 0, "hann": 1, "shepp-logan": 2, "butterworth": 3}[filter], _ptr(out), _stream(sinogram)))
         return out
 
     def mbir(self, sinogram, prior, iters, out=None):

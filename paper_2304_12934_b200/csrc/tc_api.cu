@@ -35,7 +35,7 @@ struct tc_plan {
     DevPlan d;
     int max_slab;                 // slices per slab (multiple of 8), 0 = not yet decided
     // device tables
-    float2 *twG = nullptr, *twD = nullptr, *ph_fwd = nullptr, *ph_adj = nullptr, *ph_fbp[2] = {nullptr, nullptr};
+    float2 *twG = nullptr, *twD = nullptr, *ph_fwd = nullptr, *ph_adj = nullptr, *ph_fbp[4] = {nullptr, nullptr, nullptr, nullptr};
     int fbp_filter = -1;          // >= 0 only while tc_fbp runs: index into ph_fbp
     float *deapod = nullptr, *th_sorted = nullptr;
     double2 *cs = nullptr, *cs_sorted = nullptr;
@@ -189,11 +189,11 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
         for (int i = 0; i < len; ++i) { const double a = 2.0 * M_PI * i / len; t[i] = make_float2((float)std::cos(a), (float)-std::sin(a)); }
         return t;
     };
-    std::vector<float2> phf(nd), pha(nd), phr(nd), phh(nd);       // forward / adjoint phases; adjoint x FBP weights (ramp, Hann)
+    std::vector<float2> phf(nd), pha(nd), phr(nd), phh(nd), phs(nd), phb(nd);   // forward / adjoint phases; adjoint x FBP weights (ramp, Hann, Shepp-Logan, Butterworth)
     const double centre = p->geom.center;
     for (int k = 0; k < nd; ++k) {
         const int m = k < nd / 2 ? k : k - nd;
-        if (k == nd / 2) { phf[k] = pha[k] = phr[k] = phh[k] = make_float2(0.f, 0.f); continue; }
+        if (k == nd / 2) { phf[k] = pha[k] = phr[k] = phh[k] = phs[k] = phb[k] = make_float2(0.f, 0.f); continue; }
         const double a = 2.0 * M_PI * std::fmod((double)m * centre, (double)nd) / nd;
         phf[k] = make_float2((float)(std::cos(a) / nd), (float)(-std::sin(a) / nd));
         pha[k] = make_float2((float)(std::cos(a) / nd), (float)(std::sin(a) / nd));
@@ -202,6 +202,10 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
             const double hann = ramp * 0.5 * (1.0 + std::cos(2.0 * M_PI * m / nd));
             phr[k] = make_float2((float)(ramp * std::cos(a) / nd), (float)(ramp * std::sin(a) / nd));
             phh[k] = make_float2((float)(hann * std::cos(a) / nd), (float)(hann * std::sin(a) / nd));
+            const double xs = M_PI * m / nd, shepp = ramp * (m == 0 ? 1.0 : std::sin(xs) / xs);           // filters of P:L68
+            const double butter = ramp / (1.0 + std::pow(std::fabs((double)m) / (nd / 4.0), 4.0));
+            phs[k] = make_float2((float)(shepp * std::cos(a) / nd), (float)(shepp * std::sin(a) / nd));
+            phb[k] = make_float2((float)(butter * std::cos(a) / nd), (float)(butter * std::sin(a) / nd));
         }
     }
     std::vector<double2> cs(na), css(na);
@@ -225,6 +229,8 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
     if (e == cudaSuccess) e = upload(&p->ph_adj, pha);
     if (e == cudaSuccess) e = upload(&p->ph_fbp[0], phr);
     if (e == cudaSuccess) e = upload(&p->ph_fbp[1], phh);
+    if (e == cudaSuccess) e = upload(&p->ph_fbp[2], phs);
+    if (e == cudaSuccess) e = upload(&p->ph_fbp[3], phb);
     if (e == cudaSuccess) e = upload(&p->deapod, deapod);
     if (e == cudaSuccess) e = upload(&p->cs, cs);
     if (e == cudaSuccess) e = upload(&p->cs_sorted, css);
@@ -386,7 +392,7 @@ static void free_scratch(tc_plan *p) {
 extern "C" tc_status tc_plan_destroy(tc_plan *p) {
     if (!p) return TC_OK;
     free_scratch(p);
-    cudaFree(p->twG); cudaFree(p->twD); cudaFree(p->ph_fwd); cudaFree(p->ph_adj); cudaFree(p->ph_fbp[0]); cudaFree(p->ph_fbp[1]); cudaFree(p->deapod);
+    cudaFree(p->twG); cudaFree(p->twD); cudaFree(p->ph_fwd); cudaFree(p->ph_adj); cudaFree(p->ph_fbp[0]); cudaFree(p->ph_fbp[1]); cudaFree(p->ph_fbp[2]); cudaFree(p->ph_fbp[3]); cudaFree(p->deapod);
     cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc); cudaFree(p->tile_rng); cudaFree(p->tile_nr); cudaFree(p->tap_offs); cudaFree(p->taps); cudaFree(p->heavy);
     cudaFree(p->gt_tiles); cudaFree(p->gt_start); cudaFree(p->gt_samples);
     if (p->d.side) cudaStreamDestroy(p->d.side);

@@ -145,7 +145,7 @@ extern "C" tc_status tc_backproject(tc_plan *p, const float *sinogram, int n_sli
 
 extern "C" tc_status tc_fbp(tc_plan *p, const float *sinogram, int n_slices, int filter, float *volume, void *stream) {
     if (!p) return fail(TC_EINVAL, "null plan");
-    if (filter != TC_FILTER_RAMP && filter != TC_FILTER_HANN) return fail(TC_EINVAL, "unknown filter");
+    if (filter < TC_FILTER_RAMP || filter > TC_FILTER_BUTTERWORTH) return fail(TC_EINVAL, "unknown filter");
     p->fbp_filter = filter;                                   // launches read it while they are enqueued (below), not later
     const tc_status s = run_op(p, adjoint_slab, sinogram, (size_t)p->d.na * p->d.nd, volume, (size_t)p->d.n * p->d.n, n_slices, stream);
     p->fbp_filter = -1;

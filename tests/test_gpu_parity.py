@@ -389,7 +389,7 @@ def test_fbp_vs_oracle(tc):
     ang = inputs.angles_uniform(na); a64 = ang.astype(np.float64)
     y = rng.standard_normal((S, na, nd)).astype(np.float32)
     plan = tc.Plan(n, nd, ang, centre)
-    for w in ("ramp", "hann"):
+    for w in ("ramp", "hann", "shepp-logan", "butterworth"):
         f = _np(plan.fbp(_cuda(y), w))
         assert rel_l2(f, fbp.fbp_nufft(y, a64, n, centre, w)) < TOL_NUFFT
         assert rel_l2(f[1], fbp.fbp_direct(y[1], a64, n, centre, w)) < TOL_DIRECT

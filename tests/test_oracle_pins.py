@@ -392,6 +392,11 @@ def test_fbp_hann_window_read_off_a_single_radial_mode():
         assert rel_l2(ramp, plain * (np.pi / na) * (m0 / nd)) < 1e-12
         assert rel_l2(hann, ramp * win) < 1e-12
         assert rel_l2(fbp.fbp_nufft(p, ang, n, centre, "hann"), hann) < 2e-5
+        # Shepp-Logan sin(x)/x at x = pi m0/Nd and Butterworth 1/(1 + (4 m0/Nd)^4), written out here with math, not numpy's sinc
+        x = math.pi * m0 / nd
+        assert rel_l2(fbp.fbp_direct(p, ang, n, centre, "shepp-logan"), ramp * (math.sin(x) / x)) < 1e-12
+        assert rel_l2(fbp.fbp_direct(p, ang, n, centre, "butterworth"), ramp / (1.0 + (4.0 * m0 / nd) ** 4)) < 1e-12
+    assert abs(fbp.ramp_weights(nd, na, "butterworth")[nd // 2 - 1 + 12] / fbp.ramp_weights(nd, na, "ramp")[nd // 2 - 1 + 12] - 0.5) < 1e-15   # half power at the cut-off m = Nd/4
     p0 = np.ones((na, nd))                                          # m0 = 0: DC bin, weight 1/(4 Nd), Hann = 1
     assert rel_l2(fbp.fbp_direct(p0, ang, n, centre, "hann"), direct.backproject_direct(p0, ang, n, centre) * (np.pi / na) * 0.25 / nd) < 1e-12
 
