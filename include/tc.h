@@ -47,7 +47,9 @@ typedef struct {
 } tc_geom;
 
 /* qGGMRF prior h = (|D|/sigma)^2 / (c + (|D|/sigma)^(2-p)), eq. (13); paper's values
- * p = 1.2, sigma = 1/0.7, c = 1e-4.  lambda multiplies the prior (extension, default 1).
+ * p = 1.2, sigma = 1/0.7, c = 1e-4; 1 <= p <= 2.  p = 1 is the smoothed total variation:
+ * h = u^2 / (c + u) = u - c + c^2 / (c + u), i.e. |D|/sigma up to a constant for |D| >> c sigma, still twice differentiable at 0.
+ * lambda multiplies the prior (extension, default 1).
  * L is the step constant of the fixed 1/L step; 0 means: estimated by the library (power iteration
  * on A^T A plus the curvature bound of the prior, reading G15).  nonneg != 0 adds the constraint f >= 0 (P:L24:
  * "the choice of the constraint is not limited by the algorithm design"): the candidate is projected, z = max(y - g/L, 0).

@@ -189,8 +189,8 @@ extern "C" tc_status tc_preprocess(const float *proj, const float *flat, const f
 // ---- prior test hook ---------------------------------------------------------------------------------
 static tc_status check_prior(const tc_prior *pr) {
     if (!pr) return fail(TC_EINVAL, "null prior");
-    if (!(pr->p > 1.f && pr->p <= 2.f) || !(pr->sigma > 0.f) || !(pr->c > 0.f) || !(pr->lambda >= 0.f) || !(pr->L >= 0.f))
-        return fail(TC_EINVAL, "prior: need 1 < p <= 2, sigma > 0, c > 0, lambda >= 0, L >= 0");
+    if (!(pr->p >= 1.f && pr->p <= 2.f) || !(pr->sigma > 0.f) || !(pr->c > 0.f) || !(pr->lambda >= 0.f) || !(pr->L >= 0.f))
+        return fail(TC_EINVAL, "prior: need 1 <= p <= 2, sigma > 0, c > 0, lambda >= 0, L >= 0");
     if (pr->neighbours != 0 && pr->neighbours != 26 && pr->neighbours != 10 && pr->neighbours != 6)
         return fail(TC_EINVAL, "prior: neighbours must be 26 (or 0 = 26), 10 or 6");
     return TC_OK;

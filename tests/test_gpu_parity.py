@@ -151,7 +151,7 @@ def test_prior_kernels_vs_oracle(tc):
     for shape in ((1, 32, 32), (5, 64, 96)[:1] + (40, 40), (3, 33, 33)):
         v = (rng.standard_normal(shape) * rng.choice([0.01, 1.0, 30.0])).astype(np.float32)
         v[0, :4, :4] = 0.25                                                    # flat patch: h'(0) = 0 exactly
-        for pp, ss, cc in ((P, SIG, C), (2.0, 1.0, 1.0)):                      # p = 2: the exponent 2 - p is 0 (u^0 at u = 0)
+        for pp, ss, cc in ((P, SIG, C), (2.0, 1.0, 1.0), (1.0, 0.5, 1e-3)):    # p = 2: the exponent 2 - p is 0 (u^0 at u = 0); p = 1: smoothed TV
             val, g = tc.prior_eval(_cuda(v), tc.prior_params(pp, ss, cc))
             assert abs(val - prior.H(v, pp, ss, cc)) <= 2e-6 * prior.H(v, pp, ss, cc)
             assert rel_l2(_np(g), prior.gradH(v, pp, ss, cc)) < 1e-5
@@ -265,7 +265,7 @@ def test_mbir_host_pointers_and_default_L(tc):
     assert np.array_equal(xh, _np(xd)) and [l["F"] for l in logh] == [l["F"] for l in logd]
     with pytest.raises(tc.TcError):
         plan2 = tc.Plan(64, 64, ang, 32.0)
-        plan2.mbir(_cuda(b), tc.prior_params(0.9, SIG, C), 1)                 # p outside (1, 2]
+        plan2.mbir(_cuda(b), tc.prior_params(0.9, SIG, C), 1)                 # p outside [1, 2]
 
 
 def test_full_size_config4_timed_launch_configuration(tc):
@@ -582,7 +582,7 @@ def test_prior_neighbour_sets_vs_oracle(tc):
         tc.prior_eval(_cuda(v[:, :40, :40].copy()), tc.prior_params(P, SIG, C, neighbours=18))
 
 
-@pytest.mark.parametrize("kw", [dict(neighbours=10), dict(mm_step=True), dict(mm_step=True, neighbours=6, nonneg=True)])
+@pytest.mark.parametrize("kw", [dict(neighbours=10), dict(mm_step=True), dict(mm_step=True, neighbours=6, nonneg=True), dict(p=1.0)])
 def test_mbir_variants_vs_oracle(tc, kw):
     # 11 slices of 64^2 (two groups), noisy data; the variant's flag goes to both sides; alpha is compared where it is logged
     from paper_2304_12934_b200 import inputs
@@ -591,10 +591,12 @@ def test_mbir_variants_vs_oracle(tc, kw):
     ang = inputs.angles_uniform(na); a64 = ang.astype(np.float64)
     b = (nufft.radon_nufft(inputs.volume_cfg2(S=S, n=n) - (0.25 if kw.get("nonneg") else 0.0), a64, n, centre)
          + 0.02 * np.random.default_rng(41).standard_normal((S, na, n))).astype(np.float32)
-    L, _ = mbir.lipschitz(n, a64, n, centre, P, SIG, C, 1.0)
-    xo, logo = mbir.mbir(b, a64, n, centre, P, SIG, C, 1.0, L, iters, **kw)
+    kw = dict(kw)
+    pp = kw.pop("p", P)                                                   # p = 1: smoothed total variation (8(f) row 4)
+    L, _ = mbir.lipschitz(n, a64, n, centre, pp, SIG, C, 1.0)
+    xo, logo = mbir.mbir(b, a64, n, centre, pp, SIG, C, 1.0, L, iters, **kw)
     plan = tc.Plan(n, n, ang, centre)
-    x, log = plan.mbir(_cuda(b), tc.prior_params(P, SIG, C, 1.0, L, **kw), iters)
+    x, log = plan.mbir(_cuda(b), tc.prior_params(pp, SIG, C, 1.0, L, **kw), iters)
     x = _np(x); plan.close()
     assert [l["accepted"] for l in log] == [l["accepted"] for l in logo]
     assert rel_l2(x, xo) < TOL_MBIR

@@ -519,3 +519,22 @@ def test_preprocess_inverts_beer_lambert_and_reorders():
     assert np.allclose(preprocess.preprocess(np.exp(-b).transpose(1, 0, 2)), b, atol=1e-12)
     proj[2, 1, 3] = dark[1, 3]                                                 # a dead pixel
     assert preprocess.preprocess(proj, flat, dark, floor=1e-4)[1, 2, 3] == -np.log(1e-4)
+
+
+def test_prior_p1_is_smoothed_total_variation():
+    # SURVEY 8(f) row 4 (plain TV): eq. (13) at p = 1 is h = u^2 / (c + u) = |u| - c + c^2 / (c + |u|): total variation up to a constant
+    # for |D| >> c sigma.  Pins: the algebraic identity, and H of a step of height a across one z-plane of an N^3 cube as c -> 0:
+    # the crossing pairs are N^2 faces, 4 N (N - 1) edges and 4 (N - 1)^2 corners, each |a| / sigma times its weight.
+    from oracle import prior
+    rng = np.random.default_rng(51)
+    D = rng.standard_normal(200) * 3.0
+    sig, c = 0.7, 1e-3
+    u = np.abs(D) / sig
+    assert np.max(np.abs(prior.h(D, 1.0, sig, c) - (u - c + c * c / (c + u)))) < 1e-14
+    N, a = 6, 0.8
+    f = np.zeros((N, N, N)); f[3:] = a
+    w_face, w_edge, w_corn = prior.weight((1, 0, 0)), prior.weight((1, 1, 0)), prior.weight((1, 1, 1))
+    tv = (a / sig) * (N * N * w_face + 4 * N * (N - 1) * w_edge + 4 * (N - 1) ** 2 * w_corn)
+    assert abs(prior.H(f, 1.0, sig, 1e-12) - tv) < 1e-9 * tv
+    # and the gradient is the sign pattern of TV away from zero differences: h'(D) -> sign(D) / sigma
+    assert np.max(np.abs(prior.dh(D[np.abs(D) > 0.5], 1.0, sig, 1e-12) - np.sign(D[np.abs(D) > 0.5]) / sig)) < 1e-9
