@@ -34,8 +34,8 @@ typedef enum { TC_OK = 0, TC_EINVAL = 1, TC_ENOMEM = 2, TC_ECUDA = 3, TC_EUNSUPP
 
 /* Acquisition geometry.  n: image side (even); n_det: detector bins (even); angles: HOST pointer to
  * n_angles float32 radians (copied at plan creation; any finite values); center: rotation-axis
- * position in bins (< 0 means n_det/2); oversamp must be 2.0 and kb_width 6 (Kaiser-Bessel
- * window; w ~ log10(1/eps)).  Sizes (else TC_EUNSUPPORTED): n must be a multiple of 32; n and n_det (even) must
+ * position in bins (< 0 means n_det/2); oversamp must be 2.0; kb_width = 4, 6 or 8 taps per axis of the Kaiser-Bessel
+ * window (w ~ log10(1/eps): about 3e-4, 3e-6 and 4e-8 against the direct DFT in exact arithmetic).  Sizes (else TC_EUNSUPPORTED): n must be a multiple of 32; n and n_det (even) must
  * factor into 2, 3, 5, 7 and 17 with at most five FFT passes (one per 16, per remaining power of two and per odd factor), e.g.
  * 2048, 2560 = 2^9 5, and the 2448 = 2^4 3^2 17 detector bins of the paper's Table 1 on an n = 2560 image; at most 6800. */
 typedef struct {

@@ -114,11 +114,11 @@ def prior_params(p=1.2, sigma=1 / 0.7, c=1e-4, lam=1.0, L=0.0, nonneg=False, gra
 class Plan:
     """tc_plan_create / tc_plan_destroy; methods are the C calls of the same names."""
 
-    def __init__(self, n, n_det, angles, center=-1.0, max_slab_slices=0):
+    def __init__(self, n, n_det, angles, center=-1.0, max_slab_slices=0, kb_width=6):
         ang = np.ascontiguousarray(np.asarray(angles, dtype=np.float32))
         self.n, self.n_det, self.n_angles = int(n), int(n_det), int(ang.size)
         g = tc_geom(self.n, self.n_det, self.n_angles, ang.ctypes.data_as(ctypes.POINTER(ctypes.c_float)),
-                    float(center), 2.0, 6)
+                    float(center), 2.0, int(kb_width))
         self._h = _vp()
         _check(lib.tc_plan_create(ctypes.byref(g), int(max_slab_slices), ctypes.byref(self._h)))
 

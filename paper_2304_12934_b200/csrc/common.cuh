@@ -5,7 +5,7 @@
 
 namespace tc {
 
-constexpr int KB_W = 6;          // Kaiser-Bessel window width (taps per axis)
+constexpr int KB_W = 6;          // default Kaiser-Bessel window width (taps per axis); plans take 4, 6 or 8 (DevPlan::W)
 constexpr int KB_DEG = 12;       // degree of the window polynomial in z = 2 q - 1, q = 1 - (2 r / W)^2
 constexpr unsigned SPREAD_HEAVY = 96;   // tap lists longer than this are handled by one warp per cell (k_adj_spread_heavy)
 constexpr int P = 4;             // complex planes interleaved per fine-grid cell (= 8 real slices, 32 B)
@@ -15,6 +15,10 @@ struct TileRange { int start, count, shx, shy; };   // angles (sorted order) who
 // Everything the kernels need, passed by value.
 struct DevPlan {
     int n, nd, na, G;
+    int W;                        // window width (taps per axis): 4, 6 or 8; hw = W / 2
+    double hw; float hwf;
+    int discR;                    // fine-grid cells farther than this from the origin are never touched: G / 2 + W - 1
+    float kb[KB_DEG + 1], kbs;    // window polynomial (monomial in z, c[0] + c[1] z + ...) and -2 / (W/2)^2: z = 1 - 2 (r / (W/2))^2; per plan
     double sc;                    // G / nd: fine-grid cells per radial mode
     FftDesc fN, fD;               // FFT descriptors for length n (half of the fine grid: pruned split) and nd (radial)
     const float2 *twG, *twD;      // twiddles e^{-2 pi i k / G} (length G; the length-n transforms use every 2nd) and e^{-2 pi i k / nd}
@@ -45,7 +49,7 @@ struct DevPlan {
 
 // Tile geometry of the binned gather: a tile owns the samples whose first tap (bx, by) falls into a GT_BX x GT_BY block of
 // fine-grid cells (x = the grid's fast, parity-split axis) and stages GT_CX x GT_CY cells (block + the W - 1 = 5 cells the
-// taps reach beyond it, rounded up to even) in shared memory, GT_NBUF tiles deep.
+// taps reach beyond it, rounded up to even) in shared memory, GT_NBUF tiles deep (GtDim<W>).
 #ifndef GT_BX
 #define GT_BX 90
 #endif
@@ -55,14 +59,13 @@ struct DevPlan {
 #ifndef GT_NBUF
 #define GT_NBUF 2
 #endif
-constexpr int GT_CX = (GT_BX + 5 + 1) / 2 * 2, GT_CY = GT_BY + 5;
+template <int W> struct GtDim { static constexpr int CX = (GT_BX + W - 1 + 1) / 2 * 2, CY = GT_BY + W - 1; };
 static_assert(GT_BX % 2 == 0, "tile origins must keep the parity of the fast axis");
-__host__ __device__ inline int gt_min(int G) { return -G / 2 - 4; }            // centred coordinate of tile 0's first cell (even)
-__host__ __device__ inline int gt_ntx(int G) { return (G + 8 + GT_BX - 1) / GT_BX; }
-__host__ __device__ inline int gt_nty(int G) { return (G + 8 + GT_BY - 1) / GT_BY; }
+__host__ __device__ inline int gt_pad(int W) { return (W / 2 + 1) & ~1; }      // first taps lie in [-G/2 - W/2, G/2 - W/2]; tile 0 starts on an even cell
+__host__ __device__ inline int gt_min(int G, int W) { return -G / 2 - gt_pad(W); }   // centred coordinate of tile 0's first cell (even)
+__host__ __device__ inline int gt_ntx(int G, int W) { return (G + 2 * gt_pad(W) + GT_BX - 1) / GT_BX; }
+__host__ __device__ inline int gt_nty(int G, int W) { return (G + 2 * gt_pad(W) + GT_BY - 1) / GT_BY; }
 
-// Window polynomial coefficients (monomial in z, c[0] + c[1] z + ...), set by the plan.
-void set_kb_coeffs(const float *h);
 // Roots of unity of the odd FFT radices (constant memory), set by the plan.
 void set_fft_roots();
 

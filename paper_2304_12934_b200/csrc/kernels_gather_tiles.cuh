@@ -17,8 +17,8 @@ struct GtGeom { int bx, by; float rx, ry; };
 // first tap and offsets of sample (a, m), decided in float64 exactly as k_fwd_gather / the oracle decide them (readings G6, G19)
 __device__ __forceinline__ GtGeom gt_geom(const DevPlan &d, int a, int m) {
     const double2 cs = d.cs[a];
-    const double kx = m * cs.x, ky = m * cs.y;
-    const double bxd = ceil(kx - 3.0), byd = ceil(ky - 3.0);
+    const double kx = __dmul_rn((double)m, cs.x), ky = __dmul_rn((double)m, cs.y);      // rounded products: the same kappa as the spread's lists (enum_cell_taps)
+    const double bxd = ceil(kx - d.hw), byd = ceil(ky - d.hw);
     GtGeom g; g.bx = (int)bxd; g.by = (int)byd; g.rx = (float)(kx - bxd); g.ry = (float)(ky - byd);
     return g;
 }
@@ -30,7 +30,7 @@ __global__ void k_gt_keys(DevPlan d, unsigned long long *__restrict__ keys) {
     const int a = (int)(i / d.nd), mi = (int)(i - (size_t)a * d.nd), m = mi - d.nd / 2;
     if (m == -d.nd / 2) { keys[i] = ~0ull; return; }
     const GtGeom g = gt_geom(d, a, m);
-    const int tx = (g.bx - gt_min(d.G)) / GT_BX, ty = (g.by - gt_min(d.G)) / GT_BY;
+    const int tx = (g.bx - gt_min(d.G, d.W)) / GT_BX, ty = (g.by - gt_min(d.G, d.W)) / GT_BY;
     keys[i] = ((unsigned long long)(ty * d.gt_ntx + tx) << 32) | (unsigned)(a * d.nd + (m < 0 ? m + d.nd : m));
 }
 
@@ -43,7 +43,7 @@ __global__ void k_gt_fill(DevPlan d, const unsigned long long *__restrict__ keys
     const int a = idx / d.nd, k = idx - a * d.nd, m = k < d.nd / 2 ? k : k - d.nd;
     const GtGeom g = gt_geom(d, a, m);
     const int tx = tile % d.gt_ntx, ty = tile / d.gt_ntx;
-    const int lx = g.bx - (gt_min(d.G) + tx * GT_BX), ly = g.by - (gt_min(d.G) + ty * GT_BY);   // in [0, GT_BX) x [0, GT_BY)
+    const int lx = g.bx - (gt_min(d.G, d.W) + tx * GT_BX), ly = g.by - (gt_min(d.G, d.W) + ty * GT_BY);   // in [0, GT_BX) x [0, GT_BY)
     samples[i] = make_int4(idx, (ly << 16) | lx, __float_as_int(g.rx), __float_as_int(g.ry));
     atomicAdd(&counts[tile], 1u);
 }
@@ -78,23 +78,28 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // The kernel's x is the fine grid's FAST (contiguous, parity-split) axis and y its slow axis (rows), as in k_fwd_gather.
 // Shared tile: cell (yl, xl) at ((yl * 2 + (xl & 1)) * (GT_CX / 2) + (xl >> 1)) * 32 bytes: the global row layout, cut to the tile.
 constexpr int GT_THREADS = 1024;
-constexpr int GT_RUNS = GT_CY * 2;                           // (row, parity) runs of GT_CX / 2 cells each
-constexpr int GT_RUN_BYTES = (GT_CX / 2) * 32;
-constexpr int GT_TILE_BYTES = GT_CX * GT_CY * 32;
-static_assert(GT_RUNS <= GT_THREADS, "one thread per run");
-static_assert(GT_NBUF * GT_TILE_BYTES + 64 <= 227 * 1024, "tiles must fit in shared memory");
+template <int W> struct GtT {
+    static constexpr int CX = GtDim<W>::CX, CY = GtDim<W>::CY;
+    static constexpr int RUNS = CY * 2;                      // (row, parity) runs of CX / 2 cells each
+    static constexpr int RUN_BYTES = (CX / 2) * 32;
+    static constexpr int TILE_BYTES = CX * CY * 32;
+    static_assert(RUNS <= GT_THREADS, "one thread per run");
+    static_assert(GT_NBUF * TILE_BYTES + 64 <= 227 * 1024, "tiles must fit in shared memory");
+};
 
+template <int W>
 __device__ __forceinline__ void gt_issue_tile(const DevPlan &d, const float2 *__restrict__ grid, int tile, int g, char *buf,
                                               unsigned long long *bar) {
-    // threads 0 .. GT_RUNS-1: one run each (two copies when the run wraps around the end of the parity block)
+    // threads 0 .. RUNS-1: one run each (two copies when the run wraps around the end of the parity block)
+    constexpr int GT_CX = GtT<W>::CX, GT_RUNS = GtT<W>::RUNS, GT_RUN_BYTES = GtT<W>::RUN_BYTES;
     const int r = threadIdx.x;
     if (r >= GT_RUNS) return;
     const int G = d.G, nh = G >> 1;
     const int tx = tile % d.gt_ntx, ty = tile / d.gt_ntx;
     const int yl = r >> 1, par = r & 1;
-    int Y = gt_min(G) + ty * GT_BY + yl;                                    // centred row -> storage row (taps wrap modulo G, reading G7)
+    int Y = gt_min(G, W) + ty * GT_BY + yl;                                    // centred row -> storage row (taps wrap modulo G, reading G7)
     Y %= G; if (Y < 0) Y += G;
-    int X = gt_min(G) + tx * GT_BX + par;                                   // first cell of the run (centred; same parity as par)
+    int X = gt_min(G, W) + tx * GT_BX + par;                                   // first cell of the run (centred; same parity as par)
     X %= G; if (X < 0) X += G;
     const int pos0 = X >> 1;
     const int len1 = min(GT_CX / 2, nh - pos0), len2 = GT_CX / 2 - len1;
@@ -134,19 +139,23 @@ __device__ __forceinline__ void gt_advance(const DevPlan &d, int ng, GtCursor &c
     gt_decode(d, ng, c);
 }
 
-struct GtTaps { float wx[KB_W], wy[KB_W]; int base; };          // window weights and the float4 index of tap (0, 0) in the tile
-__device__ __forceinline__ GtTaps gt_taps(const int4 e) {
-    GtTaps t;
+template <int W> struct GtTaps { float wx[W], wy[W]; int base; };          // window weights and the float4 index of tap (0, 0) in the tile
+template <int W>
+__device__ __forceinline__ GtTaps<W> gt_taps(const DevPlan &d, const int4 e) {
+    constexpr int KB_W = W, GT_CX = GtT<W>::CX;
+    GtTaps<W> t;
     const int lx = e.y & 0xffff, ly = e.y >> 16;
     const float rx = __int_as_float(e.z), ry = __int_as_float(e.w);
 #pragma unroll
-    for (int k = 0; k < KB_W; ++k) { t.wx[k] = kb_eval(rx - (float)k); t.wy[k] = kb_eval(ry - (float)k); }
+    for (int k = 0; k < KB_W; ++k) { t.wx[k] = kb_eval(d, rx - (float)k); t.wy[k] = kb_eval(d, ry - (float)k); }
     // cell (yl, xl) sits at float4 index (yl * GT_CX + (xl & 1) * (GT_CX / 2) + (xl >> 1)) * 2: taps t and t + 2 along x are neighbours
     t.base = (ly * GT_CX + (lx & 1) * (GT_CX / 2) + (lx >> 1)) * 2;
     return t;
 }
-// sum over the 6 x 6 taps; `odd` = parity of the first tap's column (decides on which side of the parity split taps 1, 3, 5 lie)
-__device__ __forceinline__ float4 gt_apply(const float4 *__restrict__ tb, const GtTaps &t, bool odd) {
+// sum over the W x W taps; `odd` = parity of the first tap's column (decides on which side of the parity split taps 1, 3, 5 lie)
+template <int W>
+__device__ __forceinline__ float4 gt_apply(const float4 *__restrict__ tb, const GtTaps<W> &t, bool odd) {
+    constexpr int KB_W = W, GT_CX = GtT<W>::CX;
     // x taps 0, 2, 4 share the parity of lx and sit at +0, +1, +2 cells; taps 1, 3, 5 have the other parity: the other run, and one cell
     // further along when lx is odd
     const int o1 = odd ? (1 - GT_CX / 2) * 2 : (GT_CX / 2) * 2;
@@ -165,7 +174,9 @@ __device__ __forceinline__ float4 gt_apply(const float4 *__restrict__ tb, const 
     return acc;
 }
 
+template <int W>
 __global__ void __launch_bounds__(GT_THREADS, 1) k_fwd_gather_tiles(DevPlan d, const float2 *__restrict__ grid, int ng, float2 *__restrict__ cpol) {
+    constexpr int GT_RUNS = GtT<W>::RUNS, GT_TILE_BYTES = GtT<W>::TILE_BYTES;
     extern __shared__ __align__(128) char gt_smem[];
     char *tiles = gt_smem;                                                 // GT_NBUF x GT_TILE_BYTES
     unsigned long long *bars = reinterpret_cast<unsigned long long *>(gt_smem + GT_NBUF * GT_TILE_BYTES);
@@ -181,15 +192,15 @@ __global__ void __launch_bounds__(GT_THREADS, 1) k_fwd_gather_tiles(DevPlan d, c
     // prologue: GT_NBUF - 1 loads are on their way before the first one is read
 #pragma unroll
     for (int j = 0; j < GT_NBUF - 1; ++j)
-        if (prod.valid) { gt_issue_tile(d, grid, prod.tile, prod.g0 + prod.j, tiles + j * GT_TILE_BYTES, &bars[j]); gt_advance(d, ng, prod); }
-    GtTaps mine;                                                           // this pair's first sample of the current tile, kept across its groups
+        if (prod.valid) { gt_issue_tile<W>(d, grid, prod.tile, prod.g0 + prod.j, tiles + j * GT_TILE_BYTES, &bars[j]); gt_advance(d, ng, prod); }
+    GtTaps<W> mine;                                                           // this pair's first sample of the current tile, kept across its groups
     int mine_idx = -1; bool mine_odd = false;
     unsigned s0 = 0, s1 = 0;
     for (int k = 0; cons.valid; ++k) {
         if (prod.valid) {                                                  // that buffer was released by the barrier that ended load k - 1
             fence_proxy_async();
             const int bn = (k + GT_NBUF - 1) % GT_NBUF;
-            gt_issue_tile(d, grid, prod.tile, prod.g0 + prod.j, tiles + bn * GT_TILE_BYTES, &bars[bn]);
+            gt_issue_tile<W>(d, grid, prod.tile, prod.g0 + prod.j, tiles + bn * GT_TILE_BYTES, &bars[bn]);
             gt_advance(d, ng, prod);
         }
         if (cons.j == 0) {                                                 // new tile: weights of this pair's first sample
@@ -197,19 +208,19 @@ __global__ void __launch_bounds__(GT_THREADS, 1) k_fwd_gather_tiles(DevPlan d, c
             mine_idx = -1;
             if (s0 + pair < s1) {
                 const int4 e = __ldg(&d.gt_samples[s0 + pair]);
-                mine = gt_taps(e); mine_idx = e.x; mine_odd = e.y & 1;
+                mine = gt_taps<W>(d, e); mine_idx = e.x; mine_odd = e.y & 1;
             }
         }
         const int bc = k % GT_NBUF;
         const float4 *tb = reinterpret_cast<const float4 *>(tiles + bc * GT_TILE_BYTES) + hp;
         float4 *out = reinterpret_cast<float4 *>(cpol) + (size_t)(cons.g0 + cons.j) * gstride + hp;
         mbar_wait(&bars[bc], (k / GT_NBUF) & 1);
-        if (mine_idx >= 0) out[(size_t)mine_idx * 2] = gt_apply(tb, mine, mine_odd);
+        if (mine_idx >= 0) out[(size_t)mine_idx * 2] = gt_apply<W>(tb, mine, mine_odd);
 #pragma unroll 1
         for (unsigned s = s0 + pair + GT_THREADS / 2; s < s1; s += GT_THREADS / 2) {       // crowded tiles: the further samples of this pair
             const int4 e = __ldg(&d.gt_samples[s]);
-            const GtTaps t = gt_taps(e);
-            out[(size_t)e.x * 2] = gt_apply(tb, t, e.y & 1);
+            const GtTaps<W> t = gt_taps<W>(d, e);
+            out[(size_t)e.x * 2] = gt_apply<W>(tb, t, e.y & 1);
         }
         __syncthreads();                                                   // everybody is done reading this buffer
         gt_advance(d, ng, cons);
@@ -248,14 +259,20 @@ void launch_gt_keys(const DevPlan &d, unsigned long long *keys, cudaStream_t st)
 void launch_gt_fill(const DevPlan &d, const unsigned long long *keys, unsigned nvalid, int4 *samples, unsigned *counts, cudaStream_t st) {
     k_gt_fill<<<(nvalid + 255) / 256, 256, 0, st>>>(d, keys, nvalid, samples, counts);
 }
+template <int W>
+static void launch_fwd_gather_tiles_w(const DevPlan &d, const float2 *grid, int ng, float2 *cpol, int nitems, int n_sm, cudaStream_t st) {
+    const size_t sh = GT_NBUF * GtT<W>::TILE_BYTES + 64;
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(k_fwd_gather_tiles<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh); attr = true; }
+    k_fwd_gather_tiles<W><<<std::min(n_sm, nitems), GT_THREADS, sh, st>>>(d, grid, ng, cpol);
+}
 void launch_fwd_gather_tiles(const DevPlan &d, const float2 *grid, int ng, float2 *cpol, cudaStream_t st) {
     static int n_sm = 0;
     if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
-    const size_t sh = GT_NBUF * GT_TILE_BYTES + 64;
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(k_fwd_gather_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh); attr = true; }
     const int nitems = d.gt_nh * ng + (d.gt_nm - d.gt_nh) * ((ng + 3) / 4) + (d.gt_nlive - d.gt_nm) * ((ng + 15) / 16);
     if (nitems <= 0) return;
-    k_fwd_gather_tiles<<<std::min(n_sm, nitems), GT_THREADS, sh, st>>>(d, grid, ng, cpol);
+    if (d.W == 4) launch_fwd_gather_tiles_w<4>(d, grid, ng, cpol, nitems, n_sm, st);
+    else if (d.W == 8) launch_fwd_gather_tiles_w<8>(d, grid, ng, cpol, nitems, n_sm, st);
+    else launch_fwd_gather_tiles_w<6>(d, grid, ng, cpol, nitems, n_sm, st);
     TC_COUNT_LAUNCH();
 }

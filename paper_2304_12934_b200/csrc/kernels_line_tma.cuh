@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(2 * Cfg::GROUP_THREADS, 1024 / (2 * Cfg::GROUP
     for (int line = blockIdx.x; line < nlines; line += gridDim.x, ++k) {
         const int g = line / G, xs = line - g * G, x = xs < n ? 2 * xs : 2 * (xs - n) + 1;
         float2 *out = grid + ((size_t)g * G + x) * G * 4 + c.pl;
-        const int lim = disc_limit(x, G);
+        const int lim = disc_limit(x, G, d.discR);
         mbar_wait(full, k & 1);
         line_first<R0, false>(c, cfg, [&](int t, bool lo) {
             const Wrapped w = wrapped(t, n, lo);
@@ -283,7 +283,7 @@ __global__ void __launch_bounds__(NGRP * Cfg::GROUP_THREADS, 1) k_adj_cols_tma(D
     line_pipeline<Cfg, NGRP, NBUF, 2>(lt_smem, M,
         [&](const LpTask &t, char *buf, unsigned long long *bar) {
             const int line = blockIdx.x + t.m * gridDim.x, g = line / G, x = line - g * G, p = t.phase;
-            const int lim = disc_limit(x, G);
+            const int lim = disc_limit(x, G, d.discR);
             // live cells: k <= k1 (ky = 2 k + p >= 0) and k >= k2 (ky = 2 k + p - G < 0); found with disc_live itself
             int K = (int)sqrtf((float)lim);
             while ((K + 1) * (K + 1) <= lim) ++K;
@@ -301,7 +301,7 @@ __global__ void __launch_bounds__(NGRP * Cfg::GROUP_THREADS, 1) k_adj_cols_tma(D
             const int line = blockIdx.x + t.m * gridDim.x, g = line / G, x = line - g * G, p = t.phase;
             float2 *sm = reinterpret_cast<float2 *>(buf);
             const LineCtx c = line_ctx<Cfg>(sm, d.twG);
-            const int lim = disc_limit(x, G);
+            const int lim = disc_limit(x, G, d.discR);
             float2 *out = rowbuf + ((size_t)g * G + x) * n * 4 + pl;                 // adjoint half-plane, column-major: [g][x][i]
             line_first_inplace<R0, true>(c, cfg, [&](int k, bool) { return disc_live(2 * k + p, G, lim) ? sm[k * 4 + pl] : make_float2(0.f, 0.f); });
             static_finish<true, Cfg, 1, R0>(c, cfg,

@@ -15,8 +15,6 @@
 
 namespace tc {
 
-__constant__ float c_kb[KB_DEG + 1];
-void set_kb_coeffs(const float *h) { cudaMemcpyToSymbol(c_kb, h, sizeof(float) * (KB_DEG + 1)); }
 void set_fft_roots() {
     static float2 h[FFT_MAX_ODD + 1][FFT_MAX_ODD + 1];
     for (int R = 1; R <= FFT_MAX_ODD; ++R)
@@ -62,9 +60,9 @@ template <class Cfg> __device__ __forceinline__ Cfg make_cfg(const FftDesc &f, i
 }
 
 // Only the disc of fine-grid cells within W/2 of some polar sample carries data: |kappa| < G/2, so cells with
-// kx^2 + ky^2 > (G/2 + 5)^2 (21 % of the grid) are never read by the gather nor written by the spread; the column
-// kernels neither store nor load them.  lim = (G/2 + 5)^2 - kx^2 for the column at hand.
-__device__ __forceinline__ int disc_limit(int x, int G) { const int kx = x < G / 2 ? x : x - G, R = G / 2 + 5; return R * R - kx * kx; }
+// kx^2 + ky^2 > (G/2 + W - 1)^2 (21 % of the grid) are never read by the gather nor written by the spread; the column
+// kernels neither store nor load them.  lim = discR^2 - kx^2 for the column at hand.
+__device__ __forceinline__ int disc_limit(int x, int G, int R) { const int kx = x < G / 2 ? x : x - G; return R * R - kx * kx; }
 __device__ __forceinline__ bool disc_live(int y, int G, int lim) { const int ky = y < G / 2 ? y : y - G; return ky * ky <= lim; }
 
 struct Wrapped { int img, X; };      // image index and periodic fine-grid index of wrapped sample t (lo = t < n / 2)
@@ -106,7 +104,7 @@ __global__ void TC_LB2 k_fwd_cols(DevPlan d, const float2 *__restrict__ rowbuf, 
     const int x = blockIdx.x / NH, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = Cfg::PL * (blockIdx.x % NH) + threadIdx.x % Cfg::PL;
     const float2 *in = rowbuf + ((size_t)g * n * G + (size_t)(x & 1) * n + (x >> 1)) * 4 + pl;
     float2 *out = grid + ((size_t)g * G + x) * G * 4 + pl;
-    const int lim = disc_limit(x, G);
+    const int lim = disc_limit(x, G, d.discR);
 #pragma unroll 1
     for (int p = 0; p < 2; ++p) {
         fft_line<false>(sm, cfg, d.twG,
@@ -130,7 +128,7 @@ __global__ void TC_LB2 k_adj_cols(DevPlan d, const float2 *__restrict__ grid, fl
     const int x = blockIdx.x / NH, g = blockIdx.y, n = cfg.n(), G = 2 * n, pl = Cfg::PL * (blockIdx.x % NH) + threadIdx.x % Cfg::PL;
     const float2 *in = grid + ((size_t)g * G + x) * G * 4 + pl;
     float2 *out = rowbuf + ((size_t)g * G + x) * n * 4 + pl;                 // adjoint half-plane, column-major: [g][x][i]
-    const int lim = disc_limit(x, G);
+    const int lim = disc_limit(x, G, d.discR);
 #pragma unroll 1
     for (int p = 0; p < 2; ++p) {
         fft_line<true>(sm, cfg, d.twG,

@@ -1,12 +1,12 @@
 // Included by kernels_nufft.cu inside namespace tc: polar-side kernels (F3+F4, B1, B2) and launch wrappers.
 
-// Kaiser-Bessel window phi(r), |r| <= 3 (reading G5): degree-12 polynomial in z = 2 q - 1,
-// q = 1 - (r/3)^2, fitted in float64 at plan creation (max error 3e-10 before float32 rounding).
-__device__ __forceinline__ float kb_eval(float r) {
-    const float z = fmaf(r * r, -2.f / 9.f, 1.f);
-    float acc = c_kb[KB_DEG];
+// Kaiser-Bessel window phi(r), |r| <= W/2 (reading G5): degree-12 polynomial in z = 2 q - 1,
+// q = 1 - (2 r / W)^2, fitted in float64 at plan creation (max error 3e-10 before float32 rounding).
+__device__ __forceinline__ float kb_eval(const DevPlan &d, float r) {      // coefficients ride in the plan (kernel parameter space)
+    const float z = fmaf(r * r, d.kbs, 1.f);
+    float acc = d.kb[KB_DEG];
 #pragma unroll
-    for (int k = KB_DEG - 1; k >= 0; --k) acc = fmaf(acc, z, c_kb[k]);
+    for (int k = KB_DEG - 1; k >= 0; --k) acc = fmaf(acc, z, d.kb[k]);
     return acc;
 }
 
@@ -36,13 +36,13 @@ __global__ void __launch_bounds__(GATHER_THREADS, 1) k_fwd_gather(DevPlan d, con
         const int k = m < 0 ? m + nd : m;
         float4 *dst = reinterpret_cast<float4 *>(sm + (size_t)line_input_cell(nd, R1, k) * 4) + hp;
         if (m == -nd / 2) { *dst = make_float4(0.f, 0.f, 0.f, 0.f); continue; }     // Nyquist radial mode excluded (reading G2)
-        const double kx = m * cs.x, ky = m * cs.y;            // kappa = G k_m (cos, sin), in fine-grid cells
+        const double kx = __dmul_rn((double)m, cs.x), ky = __dmul_rn((double)m, cs.y);   // kappa = G k_m (cos, sin), in fine-grid cells (rounded product, see enum_cell_taps)
         const double bxd = ceil(kx - 3.0), byd = ceil(ky - 3.0);   // first tap (reading G6)
         const float rx = (float)(kx - bxd), ry = (float)(ky - byd);   // in (2, 3]
         const int bx = (int)bxd, by = (int)byd;
         float wx[KB_W], wy[KB_W];
 #pragma unroll
-        for (int t = 0; t < KB_W; ++t) { wx[t] = kb_eval(rx - (float)t); wy[t] = kb_eval(ry - (float)t); }
+        for (int t = 0; t < KB_W; ++t) { wx[t] = kb_eval(d, rx - (float)t); wy[t] = kb_eval(d, ry - (float)t); }
         float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
         int ixs[KB_W];
 #pragma unroll
@@ -136,22 +136,23 @@ __global__ void k_tile_ranges(DevPlan d, TileRange *__restrict__ rng, int *__res
     const int X0 = bx < G / 2 ? bx : bx - G, Y0 = by < G / 2 ? by : by - G;
     const int X1 = min(X0 + 31, G / 2 - 1), Y1 = min(Y0 + 7, G / 2 - 1);
     int shx[3] = {0, 0, 0}, shy[3] = {0, 0, 0}, nx = 1, ny = 1;
-    if (X0 <= -G / 2 + 3) shx[nx++] = G;                 // taps wrap modulo G (reading G7)
-    if (X1 >= G / 2 - 4) shx[nx++] = -G;
-    if (Y0 <= -G / 2 + 3) shy[ny++] = G;
-    if (Y1 >= G / 2 - 4) shy[ny++] = -G;
+    const int hwi = d.W / 2;
+    if (X0 <= -G / 2 + hwi) shx[nx++] = G;               // taps wrap modulo G (reading G7)
+    if (X1 >= G / 2 - hwi - 1) shx[nx++] = -G;
+    if (Y0 <= -G / 2 + hwi) shy[ny++] = G;
+    if (Y1 >= G / 2 - hwi - 1) shy[ny++] = -G;
     int nr = 0;
     for (int j = 0; j < ny; ++j)
         for (int i = 0; i < nx; ++i) {
             TileRange t; t.shx = shx[i]; t.shy = shy[j];
-            tile_range(d, X0 + shx[i] - 3.0, X1 + shx[i] + 3.0, Y0 + shy[j] - 3.0, Y1 + shy[j] + 3.0, t.start, t.count);
+            tile_range(d, X0 + shx[i] - d.hw, X1 + shx[i] + d.hw, Y0 + shy[j] - d.hw, Y1 + shy[j] + d.hw, t.start, t.count);
             if (t.count > 0 && nr < 4) rng[tx * 4 + nr++] = t;
         }
     nrng[tx] = nr;
 }
 
 // Enumerates, for the cell owned by this thread, every polar sample (a, m) whose W x W footprint covers it
-// (kappa - r in (-3, 3]^2, decided in float64 exactly as the forward gather decides its tap base), and calls
+// (kappa - r in (-W/2, W/2]^2, decided in float64 exactly as the forward gather decides its tap base), and calls
 // f(a * nd + (m mod nd), phi(dx) phi(dy)).  Cell order inside a tile: warp = 8 x 4 cells.
 template <class F>
 __device__ __forceinline__ void enum_cell_taps(const DevPlan &d, const TileRange *__restrict__ rng, const int *__restrict__ nrng,
@@ -169,16 +170,18 @@ __device__ __forceinline__ void enum_cell_taps(const DevPlan &d, const TileRange
             const double2 cs = d.cs_sorted[k];
             const float cf = (float)cs.x, sf = (float)cs.y;
             const float acf = fabsf(cf), asf = fabsf(sf);
-            if (fabsf(Kxf * sf - Kyf * cf) > 3.f * (acf + asf) + 0.02f) continue;   // ray misses this cell's box
+            if (fabsf(Kxf * sf - Kyf * cf) > d.hwf * (acf + asf) + 0.02f) continue;   // ray misses this cell's box
             const float mc = acf >= asf ? Kxf / cf : Kyf / sf;
             const int m_c = __float2int_rn(mc);
             const int a = d.a_sorted[k];
             for (int j = -J - 1; j <= J + 1; ++j) {
                 const int m = m_c + j;
                 if (m < -mmax || m > mmax) continue;
-                const double dx = m * cs.x - Kx, dy = m * cs.y - Ky;
-                if (dx <= -3.0 || dx > 3.0 || dy <= -3.0 || dy > 3.0) continue;
-                f(a * nd + (m < 0 ? m + nd : m), kb_eval((float)dx) * kb_eval((float)dy));
+                // kappa as the ROUNDED product (no fused multiply-add): the count and fill passes and the forward gather must take the
+                // same decision for a sample that sits exactly on the edge of the window
+                const double dx = __dmul_rn((double)m, cs.x) - Kx, dy = __dmul_rn((double)m, cs.y) - Ky;
+                if (dx <= -d.hw || dx > d.hw || dy <= -d.hw || dy > d.hw) continue;
+                f(a * nd + (m < 0 ? m + nd : m), kb_eval(d, (float)dx) * kb_eval(d, (float)dy));
             }
         }
     }
@@ -241,7 +244,7 @@ __global__ void __launch_bounds__(512, 2) k_adj_spread(DevPlan d, const unsigned
     const unsigned t0 = offs[cidx], t1 = offs[cidx + 1];
     if (t1 - t0 > SPREAD_HEAVY) return;                          // long lists (cells near the origin) go to k_adj_spread_heavy
     if (t1 == t0) {                                              // outside the sampled disc: nobody reads the cell (see disc_live)
-        const int kf = ix < G / 2 ? ix : ix - G, ks = iy < G / 2 ? iy : iy - G, R = G / 2 + 5;
+        const int kf = ix < G / 2 ? ix : ix - G, ks = iy < G / 2 ? iy : iy - G, R = d.discR;
         if (kf * kf + ks * ks > R * R) return;
     }
     // entries past the end of the list are (sample 0, weight 0)

@@ -159,7 +159,8 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
     if ((gm->n & 1) || (gm->n_det & 1)) return fail(TC_EINVAL, "n and n_det must be even");
     for (int a = 0; a < gm->n_angles; ++a)
         if (!std::isfinite(gm->angles[a])) return fail(TC_EINVAL, "non-finite angle");
-    if (gm->oversamp != 2.0f || gm->kb_width != KB_W) return fail(TC_EUNSUPPORTED, "only oversamp = 2, kb_width = 6");
+    if (gm->oversamp != 2.0f || (gm->kb_width != 4 && gm->kb_width != 6 && gm->kb_width != 8))
+        return fail(TC_EUNSUPPORTED, "only oversamp = 2 and kb_width = 4, 6 or 8");
     if (gm->n % 32) return fail(TC_EUNSUPPORTED, "n must be a multiple of 32");
     tc_plan *p = new tc_plan();
     p->geom = *gm;
@@ -173,11 +174,11 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
     if (!make_fft_desc(n, d.fN) || !make_fft_desc(nd, d.fD)) { delete p; return fail(TC_EUNSUPPORTED, "n and n_det must be 2^a 3^b 5^c 7^d 17^e, a >= 1, with at most 5 FFT passes (and at most 6800)"); }
     if (nd / 2 - 1 > 0 && d.sc * (nd / 2 - 1) + 3 >= G / 2 + 3) { /* taps wrap at most once; always true for sc = G/nd */ }
 
-    const int W = KB_W; const double sigma = 2.0;
+    const int W = gm->kb_width; const double sigma = 2.0;
+    d.W = W; d.hw = 0.5 * W; d.hwf = 0.5f * W; d.discR = G / 2 + W - 1;
     const double beta = kb_beta(W, sigma), i0b = bessel_i0(beta);
-    float kb[KB_DEG + 1];
-    kb_poly(W, sigma, kb);
-    set_kb_coeffs(kb);
+    kb_poly(W, sigma, d.kb);
+    d.kbs = -8.f / (float)(W * W);
     set_fft_roots();
     std::vector<float> deapod(n);
     for (int j = 0; j < n; ++j) {
@@ -240,7 +241,7 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
     if (e != cudaSuccess) { tc_plan_destroy(p); return fail(e == cudaErrorMemoryAllocation ? TC_ENOMEM : TC_ECUDA, cudaGetErrorString(e)); }
     d.twG = p->twG; d.twD = p->twD; d.ph_fwd = p->ph_fwd; d.ph_adj = p->ph_adj; d.deapod = p->deapod;
     d.cs = p->cs; d.cs_sorted = p->cs_sorted; d.th_sorted = p->th_sorted; d.a_sorted = p->a_sorted;
-    d.J = (int)std::floor(3.0 * std::sqrt(2.0) / d.sc + 0.5);
+    d.J = (int)std::floor(d.hw * std::sqrt(2.0) / d.sc + 0.5);
     {
         const int nt = ((G + 31) / 32) * ((G + 7) / 8);
         e = cudaMalloc((void **)&p->tile_rng, (size_t)nt * 4 * sizeof(TileRange));
@@ -292,7 +293,7 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
     }
     {   // tile-binned gather: samples sorted by tile (radix sort of (tile, sample) keys), tile offsets, tiles ordered by load
         const size_t ns = (size_t)na * nd;
-        d.gt_ntx = gt_ntx(G); d.gt_nty = gt_nty(G);
+        d.gt_ntx = gt_ntx(G, W); d.gt_nty = gt_nty(G, W);
         const int ntile = d.gt_ntx * d.gt_nty;
         unsigned long long *keys = nullptr, *keys2 = nullptr; void *tmp = nullptr; size_t tmp_bytes = 0; unsigned *counts = nullptr;
         const int end_bit = 32 + std::max(1, (int)std::ceil(std::log2((double)ntile + 1)));
@@ -376,7 +377,7 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
         }
         d.gt_tiles = p->gt_tiles; d.gt_start = p->gt_start; d.gt_samples = p->gt_samples;
         const char *env = std::getenv("TC_GATHER");
-        p->gather_tiles = !(env && std::string(env) == "ray");
+        p->gather_tiles = !(env && std::string(env) == "ray") || W != KB_W;      // the ray-by-ray kernel is built for W = 6 only
     }
     *out = p;
     return TC_OK;

@@ -101,6 +101,29 @@ def test_shapes_and_ragged_tails(tc, S, N, Nd, Na, centre):
     assert _adj_mismatch(vol, y, s, b) < TOL_ADJ
 
 
+@pytest.mark.parametrize("W,tol_direct", [(4, 2e-3), (8, 1e-5)])
+def test_window_widths_4_and_8(tc, W, tol_direct):
+    # SURVEY 8(f) row 5 (general W): the width of the Kaiser-Bessel window is the accuracy knob of the method (w ~ log10(1/eps)).
+    # GPU vs the oracle run with the same W (same tolerance as W = 6), vs the direct DFT at the accuracy that W gives, adjoint identity;
+    # shapes: a wrap-around case (samples up to the edge of the fine grid), n_det != n, a ragged group, radix-5 sizes.
+    from oracle import nufft, direct
+    for S, N, Nd, Na, centre in ((3, 64, 64, 9, 33.5), (9, 160, 200, 12, 97.25), (2, 256, 128, 10, 60.0)):
+        rng = np.random.default_rng(100 * W + N)
+        ang = np.sort(rng.uniform(0, math.pi, Na)).astype(np.float32); a64 = ang.astype(np.float64)
+        vol = rng.random((S, N, N)).astype(np.float32); y = rng.standard_normal((S, Na, Nd)).astype(np.float32)
+        plan = tc.Plan(N, Nd, ang, centre, kb_width=W)
+        s = _np(plan.radon(_cuda(vol))); b = _np(plan.backproject(_cuda(y)))
+        plan.close()
+        assert rel_l2(s, nufft.radon_nufft(vol, a64, Nd, centre, W=W)) < TOL_NUFFT
+        assert rel_l2(b, nufft.backproject_nufft(y, a64, N, centre, W=W)) < TOL_NUFFT
+        assert _adj_mismatch(vol, y, s, b) < TOL_ADJ
+        if N == 64:
+            e = rel_l2(s, direct.radon_direct(vol, a64, Nd, centre))
+            assert e < tol_direct, e
+            if W == 4:
+                assert e > 2e-5                                       # and W does change the accuracy (3e-4 in float64): not the W = 6 path in disguise
+
+
 def test_arbitrary_angles_unsorted_negative_and_beyond_pi(tc):
     from oracle import nufft
     rng = np.random.default_rng(13)
