@@ -33,7 +33,10 @@ struct DevPlan {
     const int *tile_nr;           // [tiles] number of valid ranges
     const unsigned *tap_offs;     // [tiles * 256 + 1] CSR offsets of the spread's per-cell tap lists (cell order: tile, then thread)
     const int2 *taps;             // (a * nd + (m mod nd), float weight bits)
-    const unsigned *heavy;        // [n_heavy] cells (cidx) whose list is longer than SPREAD_HEAVY
+    const unsigned *pair_offs;    // [tiles * 128 + 1] CSR offsets of the lists of the cell pairs (k_adj_spread_pairs)
+    const int *pair_idx;          // a * nd + (m mod nd)
+    const float2 *pair_w;         // weights for cell 0 and cell 1 of the pair
+    const unsigned *heavy;        // [n_heavy] cells (cidx) whose list, or whose pair partner's, is longer than SPREAD_HEAVY
     unsigned n_heavy;
     cudaStream_t side;            // the heavy-cell kernel runs beside the main spread kernel (disjoint cells): fork / join events
     cudaEvent_t ev_fork, ev_join;
@@ -88,6 +91,8 @@ void launch_tile_ranges(const DevPlan &d, TileRange *rng, int *nrng, cudaStream_
 void launch_spread_count(const DevPlan &d, int *counts, cudaStream_t st);
 void launch_spread_fill(const DevPlan &d, cudaStream_t st);
 void launch_spread_heavy_list(const DevPlan &d, unsigned ncell, unsigned *list, unsigned *count, cudaStream_t st);
+void launch_pair_count(const DevPlan &d, unsigned *counts, cudaStream_t st);
+void launch_pair_fill(const DevPlan &d, int *pidx, float2 *pw, cudaStream_t st);
 void launch_adj_spread(const DevPlan &d, const float2 *cpol, int ng, float2 *grid, cudaStream_t st);
 // grid -> rowbuf (cropped to n rows)             (B3 inverse column FFT)
 void launch_adj_cols(const DevPlan &d, const float2 *grid, int ng, float2 *rowbuf, cudaStream_t st);

@@ -45,6 +45,7 @@ struct tc_plan {
     int2 *taps = nullptr;
     unsigned *heavy = nullptr;
     long long n_taps = 0;
+    unsigned *pair_offs = nullptr; int *pair_idx = nullptr; float2 *pair_w = nullptr;      // lists of the cell pairs
     int *gt_tiles = nullptr; unsigned *gt_start = nullptr; int4 *gt_samples = nullptr;   // tile-binned gather tables
     bool gather_tiles = true;     // F3 as k_fwd_gather_tiles + k_fwd_radial (default) or as the fused ray-by-ray k_fwd_gather (TC_GATHER=ray)
     // scratch
@@ -272,7 +273,7 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
         d.tap_offs = p->tap_offs; d.taps = p->taps;
         launch_spread_fill(d, nullptr);
         {   // cells with long lists: at most the disc of radius ~ 36 na / (2 pi SPREAD_HEAVY) cells; size the list for all cells with > SPREAD_HEAVY taps
-            const size_t cap = std::min<size_t>(nc, (size_t)total / SPREAD_HEAVY + 1);
+            const size_t cap = std::min<size_t>(nc, 2 * ((size_t)total / SPREAD_HEAVY + 1));      // long lists and their pair partners
             unsigned *cnt = nullptr;
             e = cudaMalloc((void **)&p->heavy, cap * sizeof(unsigned));
             if (e == cudaSuccess) e = cudaMalloc((void **)&cnt, sizeof(unsigned));
@@ -287,6 +288,28 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
                 if (e == cudaSuccess) e = cudaEventCreateWithFlags(&d.ev_join, cudaEventDisableTiming);
             }
             if (e != cudaSuccess) { tc_plan_destroy(p); return fail(TC_ECUDA, std::string("spread heavy list: ") + cudaGetErrorString(e)); }
+        }
+        {   // lists of the cell pairs (k_adj_spread_pairs): count, exclusive scan, fill
+            const size_t np = (size_t)nt * 128;
+            unsigned *pc = nullptr; void *tmp2 = nullptr; size_t tb2 = 0; unsigned ptotal = 0;
+            d.pair_offs = nullptr; d.pair_idx = nullptr; d.pair_w = nullptr;
+            e = cudaMalloc((void **)&pc, (np + 1) * sizeof(unsigned));
+            if (e == cudaSuccess) e = cudaMemset(pc, 0, (np + 1) * sizeof(unsigned));
+            if (e == cudaSuccess) e = cudaMalloc((void **)&p->pair_offs, (np + 1) * sizeof(unsigned));
+            if (e == cudaSuccess) {
+                launch_pair_count(d, pc, nullptr);
+                cub::DeviceScan::ExclusiveSum(nullptr, tb2, pc, p->pair_offs, (int)(np + 1));
+                e = cudaMalloc(&tmp2, tb2);
+            }
+            if (e == cudaSuccess) e = cub::DeviceScan::ExclusiveSum(tmp2, tb2, pc, p->pair_offs, (int)(np + 1));
+            if (e == cudaSuccess) e = cudaMemcpy(&ptotal, p->pair_offs + np, sizeof(unsigned), cudaMemcpyDeviceToHost);
+            cudaFree(pc); cudaFree(tmp2);
+            if (e == cudaSuccess) e = cudaMalloc((void **)&p->pair_idx, (size_t)std::max(ptotal, 1u) * sizeof(int));
+            if (e == cudaSuccess) e = cudaMalloc((void **)&p->pair_w, (size_t)std::max(ptotal, 1u) * sizeof(float2));
+            if (e != cudaSuccess) { tc_plan_destroy(p); return fail(e == cudaErrorMemoryAllocation ? TC_ENOMEM : TC_ECUDA, std::string("spread pair lists: ") + cudaGetErrorString(e)); }
+            d.pair_offs = p->pair_offs;
+            launch_pair_fill(d, p->pair_idx, p->pair_w, nullptr);
+            d.pair_idx = p->pair_idx; d.pair_w = p->pair_w;
         }
         e = cudaDeviceSynchronize();
         if (e != cudaSuccess) { tc_plan_destroy(p); return fail(TC_ECUDA, std::string("spread tap lists: ") + cudaGetErrorString(e)); }
@@ -394,7 +417,7 @@ extern "C" tc_status tc_plan_destroy(tc_plan *p) {
     if (!p) return TC_OK;
     free_scratch(p);
     cudaFree(p->twG); cudaFree(p->twD); cudaFree(p->ph_fwd); cudaFree(p->ph_adj); cudaFree(p->ph_fbp[0]); cudaFree(p->ph_fbp[1]); cudaFree(p->ph_fbp[2]); cudaFree(p->ph_fbp[3]); cudaFree(p->deapod);
-    cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc); cudaFree(p->tile_rng); cudaFree(p->tile_nr); cudaFree(p->tap_offs); cudaFree(p->taps); cudaFree(p->heavy);
+    cudaFree(p->cs); cudaFree(p->cs_sorted); cudaFree(p->th_sorted); cudaFree(p->a_sorted); cudaFree(p->acc); cudaFree(p->tile_rng); cudaFree(p->tile_nr); cudaFree(p->tap_offs); cudaFree(p->taps); cudaFree(p->heavy); cudaFree(p->pair_offs); cudaFree(p->pair_idx); cudaFree(p->pair_w);
     cudaFree(p->gt_tiles); cudaFree(p->gt_start); cudaFree(p->gt_samples);
     if (p->d.side) cudaStreamDestroy(p->d.side);
     if (p->d.ev_fork) cudaEventDestroy(p->d.ev_fork);
