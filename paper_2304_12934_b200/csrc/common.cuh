@@ -8,6 +8,9 @@ namespace tc {
 constexpr int KB_W = 6;          // default Kaiser-Bessel window width (taps per axis); plans take 4, 6 or 8 (DevPlan::W)
 constexpr int KB_DEG = 12;       // degree of the window polynomial in z = 2 q - 1, q = 1 - (2 r / W)^2
 constexpr unsigned SPREAD_HEAVY = 96;   // tap lists longer than this are handled by one warp per cell (k_adj_spread_heavy)
+#ifndef SP_NC
+#define SP_NC 2                 // cells of a run of the spread (k_adj_spread_runs): 2 or 4
+#endif
 constexpr int P = 4;             // complex planes interleaved per fine-grid cell (= 8 real slices, 32 B)
 
 struct TileRange { int start, count, shx, shy; };   // angles (sorted order) whose ray can touch a 32 x 8 tile, per wrap alias
@@ -33,9 +36,9 @@ struct DevPlan {
     const int *tile_nr;           // [tiles] number of valid ranges
     const unsigned *tap_offs;     // [tiles * 256 + 1] CSR offsets of the spread's per-cell tap lists (cell order: tile, then thread)
     const int2 *taps;             // (a * nd + (m mod nd), float weight bits)
-    const unsigned *pair_offs;    // [tiles * 128 + 1] CSR offsets of the lists of the cell pairs (k_adj_spread_pairs)
+    const unsigned *pair_offs;    // [tiles * runs per tile + 1] CSR offsets of the lists of the cell runs (k_adj_spread_runs)
     const int *pair_idx;          // a * nd + (m mod nd)
-    const float2 *pair_w;         // weights for cell 0 and cell 1 of the pair
+    const void *pair_w;           // one weight per cell of the run (SpW)
     const unsigned *heavy;        // [n_heavy] cells (cidx) whose list, or whose pair partner's, is longer than SPREAD_HEAVY
     unsigned n_heavy;
     cudaStream_t side;            // the heavy-cell kernel runs beside the main spread kernel (disjoint cells): fork / join events
@@ -92,7 +95,8 @@ void launch_spread_count(const DevPlan &d, int *counts, cudaStream_t st);
 void launch_spread_fill(const DevPlan &d, cudaStream_t st);
 void launch_spread_heavy_list(const DevPlan &d, unsigned ncell, unsigned *list, unsigned *count, cudaStream_t st);
 void launch_pair_count(const DevPlan &d, unsigned *counts, cudaStream_t st);
-void launch_pair_fill(const DevPlan &d, int *pidx, float2 *pw, cudaStream_t st);
+void launch_pair_fill(const DevPlan &d, int *pidx, void *pw, cudaStream_t st);
+int spread_run_cells();               // cells per run (2 or 4)
 void launch_adj_spread(const DevPlan &d, const float2 *cpol, int ng, float2 *grid, cudaStream_t st);
 // grid -> rowbuf (cropped to n rows)             (B3 inverse column FFT)
 void launch_adj_cols(const DevPlan &d, const float2 *grid, int ng, float2 *rowbuf, cudaStream_t st);

@@ -281,10 +281,12 @@ __global__ void __launch_bounds__(512, 2) k_adj_spread(DevPlan d, const unsigned
 // shuffle reduction, so the result stays deterministic and no thread of the main kernel runs a long serial loop.
 __global__ void k_spread_heavy_list(DevPlan d, const unsigned *__restrict__ offs, unsigned ncell, unsigned *__restrict__ list, unsigned *__restrict__ count) {
     const unsigned c = blockIdx.x * blockDim.x + threadIdx.x;
-    // a cell is listed if its own list or its pair partner's (c ^ 1: k_adj_spread_pairs) is long
+    // a cell is listed if its own list or that of a cell of the same run (k_adj_spread_runs) is long
     if (c >= ncell) return;
-    const unsigned p = c ^ 1u;
-    if (offs[c + 1] - offs[c] > SPREAD_HEAVY || offs[p + 1] - offs[p] > SPREAD_HEAVY) list[atomicAdd(count, 1u)] = c;
+    const unsigned c0 = c & ~(unsigned)(SP_NC - 1);
+    bool heavy = false;
+    for (unsigned k = c0; k < c0 + SP_NC; ++k) heavy = heavy || offs[k + 1] - offs[k] > SPREAD_HEAVY;
+    if (heavy) list[atomicAdd(count, 1u)] = c;
 }
 
 template <int GPT>
@@ -326,119 +328,160 @@ __global__ void __launch_bounds__(256) k_adj_spread_heavy(DevPlan d, const unsig
     }
 }
 
-// ---- B2 by pairs of cells (default) ----------------------------------------------------------------------------------------------
-// k_adj_spread is bound by the L1 data pipe at one 32-byte sector per tap and group.  Two cells next to each other along the fast
-// axis share five sixths of their samples, so a lane pair now owns TWO cells (ix, ix + 1, ix even) and walks the union of their
-// lists, (sample, weight for cell 0, weight for cell 1): 42 instead of 72 loads per full 6 x 6 footprint pair, the same FMAs plus
-// those with a zero weight (which leave the sum unchanged: the result is bit-identical to the per-cell form).  Lists are plan-time
-// data as before; the first 8 entries stay in registers across the groups of the slab.
+// ---- B2 by runs of cells (default) -----------------------------------------------------------------------------------------------
+// k_adj_spread is bound by the L1 data pipe at one 32-byte sector per tap and group.  SP_NC cells next to each other along the fast
+// axis share most of their samples (two cells: 42 instead of 72 per full footprint; four: 54 instead of 144), so a lane pair now
+// owns a run of SP_NC cells (ix0 .. ix0 + NC - 1, ix0 a multiple of NC) and walks the union of their lists, (sample, one weight per
+// cell): the same FMAs plus those with a zero weight, which leave the sum unchanged: the result is bit-identical to the per-cell
+// form.  Lists are plan-time data as before; the first SP_NR entries stay in registers across the groups of the slab.
+constexpr int SP_NR = SP_NC == 2 ? 8 : 6;                 // list entries kept in registers
+constexpr int SP_RUNS = 256 / SP_NC;                      // runs per 32 x 8 tile
+struct SpW { float w[SP_NC]; };
+
 template <class F>
-__device__ __forceinline__ void enum_pair_taps(const DevPlan &d, const TileRange *__restrict__ rng, const int *__restrict__ nrng,
-                                               int tile, int ix0, int iy, F f) {
+__device__ __forceinline__ void enum_run_taps(const DevPlan &d, const TileRange *__restrict__ rng, const int *__restrict__ nrng,
+                                              int tile, int ix0, int iy, F f) {
     const int G = d.G, nd = d.nd, na = d.na;
-    const int Kx0 = ix0 < G / 2 ? ix0 : ix0 - G, Ky0 = iy < G / 2 ? iy : iy - G;      // cell 1 is Kx0 + 1 (ix0 even, G / 2 even)
+    const int Kx0 = ix0 < G / 2 ? ix0 : ix0 - G, Ky0 = iy < G / 2 ? iy : iy - G;      // cell c is Kx0 + c (a run never straddles G / 2)
     const int mmax = nd / 2 - 1, J = d.J;
     const int nr = nrng[tile];
     for (int e = 0; e < nr; ++e) {
         const TileRange tr = rng[tile * 4 + e];
         const int Kx = Kx0 + tr.shx, Ky = Ky0 + tr.shy;
-        const float Kxf = (float)Kx, Kyf = (float)Ky;
+        const float Kxf = (float)Kx, Kyf = (float)Ky, Kxl = Kxf + (float)(SP_NC - 1);
         for (int i = 0; i < tr.count; ++i) {
             int k = tr.start + i; if (k >= na) k -= na;
             const double2 cs = d.cs_sorted[k];
             const float cf = (float)cs.x, sf = (float)cs.y;
             const float acf = fabsf(cf), asf = fabsf(sf);
-            const float lim = d.hwf * (acf + asf) + 0.02f;
-            if (fabsf(Kxf * sf - Kyf * cf) > lim && fabsf((Kxf + 1.f) * sf - Kyf * cf) > lim) continue;   // the ray misses both boxes
-            const float mc0 = acf >= asf ? Kxf / cf : Kyf / sf, mc1 = acf >= asf ? (Kxf + 1.f) / cf : mc0;
+            // the ray misses the box of the whole run (the boxes of the cells, widened by the run's extent along x)
+            if (fabsf((Kxf + 0.5f * (SP_NC - 1)) * sf - Kyf * cf) > d.hwf * (acf + asf) + 0.5f * (SP_NC - 1) * asf + 0.02f) continue;
+            const float mc0 = acf >= asf ? Kxf / cf : Kyf / sf, mc1 = acf >= asf ? Kxl / cf : mc0;
             const int ma = __float2int_rn(fminf(mc0, mc1)) - J - 1, mb = __float2int_rn(fmaxf(mc0, mc1)) + J + 1;
             const int a = d.a_sorted[k];
             for (int m = max(ma, -mmax); m <= min(mb, mmax); ++m) {
                 const double kx = __dmul_rn((double)m, cs.x), dy = __dmul_rn((double)m, cs.y) - Ky;       // rounded products (enum_cell_taps)
                 if (dy <= -d.hw || dy > d.hw) continue;
-                const double dx0 = kx - Kx, dx1 = kx - (Kx + 1);
-                const bool in0 = dx0 > -d.hw && dx0 <= d.hw, in1 = dx1 > -d.hw && dx1 <= d.hw;
-                if (!in0 && !in1) continue;
+                SpW w; bool any = false;
                 const float wy = kb_eval(d, (float)dy);
-                f(a * nd + (m < 0 ? m + nd : m), in0 ? kb_eval(d, (float)dx0) * wy : 0.f, in1 ? kb_eval(d, (float)dx1) * wy : 0.f);
+#pragma unroll
+                for (int c = 0; c < SP_NC; ++c) {
+                    const double dx = kx - (Kx + c);
+                    const bool in = dx > -d.hw && dx <= d.hw;
+                    w.w[c] = in ? kb_eval(d, (float)dx) * wy : 0.f;
+                    any = any || in;
+                }
+                if (any) f(a * nd + (m < 0 ? m + nd : m), w);
             }
         }
     }
 }
-// pair q of a tile (128 pairs, the order of spread_cell): cell 0 = c0, cell 1 = c0 + 1
-__device__ __forceinline__ void spread_pair(int q, int bx, int by, int &c0, int &ix0, int &iy) {
-    const int cw = q >> 4, cl = (q & 15) * 2;
+// run q of a tile (the order of spread_cell): first cell c0, cells c0 .. c0 + NC - 1
+__device__ __forceinline__ void spread_run(int q, int bx, int by, int &c0, int &ix0, int &iy) {
+    constexpr int RPW = 32 / SP_NC;                       // runs per 32 cells of spread_cell's order
+    const int cw = q / RPW, cl = (q % RPW) * SP_NC;
     c0 = cw * 32 + cl;
     ix0 = bx * 32 + (cw & 3) * 8 + (cl & 7); iy = by * 8 + (cw >> 2) * 4 + (cl >> 3);
 }
-__global__ void __launch_bounds__(128) k_pair_count(DevPlan d, unsigned *__restrict__ counts) {
-    int c0, ix0, iy; spread_pair(threadIdx.x, blockIdx.x, blockIdx.y, c0, ix0, iy);
+__global__ void __launch_bounds__(SP_RUNS) k_run_count(DevPlan d, unsigned *__restrict__ counts) {
+    int c0, ix0, iy; spread_run(threadIdx.x, blockIdx.x, blockIdx.y, c0, ix0, iy);
     const int tile = blockIdx.y * gridDim.x + blockIdx.x;
     unsigned n = 0;
-    if (ix0 < d.G && iy < d.G) enum_pair_taps(d, d.tile_rng, d.tile_nr, tile, ix0, iy, [&](int, float, float) { ++n; });
-    counts[tile * 128 + threadIdx.x] = n;
+    if (ix0 < d.G && iy < d.G) enum_run_taps(d, d.tile_rng, d.tile_nr, tile, ix0, iy, [&](int, const SpW &) { ++n; });
+    counts[tile * SP_RUNS + threadIdx.x] = n;
 }
-__global__ void __launch_bounds__(128) k_pair_fill(DevPlan d, const unsigned *__restrict__ poffs, int *__restrict__ pidx, float2 *__restrict__ pw) {
-    int c0, ix0, iy; spread_pair(threadIdx.x, blockIdx.x, blockIdx.y, c0, ix0, iy);
+__global__ void __launch_bounds__(SP_RUNS) k_run_fill(DevPlan d, const unsigned *__restrict__ poffs, int *__restrict__ pidx, SpW *__restrict__ pw) {
+    int c0, ix0, iy; spread_run(threadIdx.x, blockIdx.x, blockIdx.y, c0, ix0, iy);
     const int tile = blockIdx.y * gridDim.x + blockIdx.x;
     if (ix0 >= d.G || iy >= d.G) return;
-    unsigned o = poffs[tile * 128 + threadIdx.x];
-    enum_pair_taps(d, d.tile_rng, d.tile_nr, tile, ix0, iy, [&](int idx, float w0, float w1) { pidx[o] = idx; pw[o] = make_float2(w0, w1); ++o; });
+    unsigned o = poffs[tile * SP_RUNS + threadIdx.x];
+    enum_run_taps(d, d.tile_rng, d.tile_nr, tile, ix0, iy, [&](int idx, const SpW &w) { pidx[o] = idx; pw[o] = w; ++o; });
 }
 
 template <int GPT>
-__device__ __forceinline__ void pair_tap(const float4 *__restrict__ cg, const size_t (&qoff)[GPT], int idx, float2 w, float4 (&a0)[GPT], float4 (&a1)[GPT]) {
+__device__ __forceinline__ void run_tap(const float4 *__restrict__ cg, const size_t (&qoff)[GPT], int idx, const SpW &w, float4 (&acc)[SP_NC][GPT]) {
     const float4 *ca = cg + (size_t)idx * 2;
 #pragma unroll
     for (int k = 0; k < GPT; ++k) {
         const float4 v = __ldg(ca + qoff[k]);
-        a0[k].x = fmaf(w.x, v.x, a0[k].x); a0[k].y = fmaf(w.x, v.y, a0[k].y); a0[k].z = fmaf(w.x, v.z, a0[k].z); a0[k].w = fmaf(w.x, v.w, a0[k].w);
-        a1[k].x = fmaf(w.y, v.x, a1[k].x); a1[k].y = fmaf(w.y, v.y, a1[k].y); a1[k].z = fmaf(w.y, v.z, a1[k].z); a1[k].w = fmaf(w.y, v.w, a1[k].w);
+#pragma unroll
+        for (int c = 0; c < SP_NC; ++c) {
+            acc[c][k].x = fmaf(w.w[c], v.x, acc[c][k].x); acc[c][k].y = fmaf(w.w[c], v.y, acc[c][k].y);
+            acc[c][k].z = fmaf(w.w[c], v.z, acc[c][k].z); acc[c][k].w = fmaf(w.w[c], v.w, acc[c][k].w);
+        }
     }
+}
+__device__ __forceinline__ SpW spw_load(const SpW *p) {
+    SpW w;
+    if constexpr (SP_NC == 2) { const float2 t = __ldg(reinterpret_cast<const float2 *>(p)); w.w[0] = t.x; w.w[1] = t.y; }
+    else { const float4 t = __ldg(reinterpret_cast<const float4 *>(p)); w.w[0] = t.x; w.w[1] = t.y; w.w[SP_NC - 2] = t.z; w.w[SP_NC - 1] = t.w; }
+    return w;
 }
 
 template <int GPT>
-__global__ void __launch_bounds__(256, 3) k_adj_spread_pairs(DevPlan d, const unsigned *__restrict__ offs, const unsigned *__restrict__ poffs,
-                                                             const int *__restrict__ pidx, const float2 *__restrict__ pw,
-                                                             const float2 *__restrict__ cpol, int ng, float2 *__restrict__ grid) {
+__global__ void __launch_bounds__(2 * SP_RUNS, SP_NC == 2 ? 3 : 4) k_adj_spread_runs(DevPlan d, const unsigned *__restrict__ offs, const unsigned *__restrict__ poffs,
+                                                            const int *__restrict__ pidx, const SpW *__restrict__ pw,
+                                                            const float2 *__restrict__ cpol, int ng, float2 *__restrict__ grid) {
     const int q = threadIdx.x >> 1, hp = threadIdx.x & 1, G = d.G;
-    int c0, ix0, iy; spread_pair(q, blockIdx.x, blockIdx.y, c0, ix0, iy);
+    int c0, ix0, iy; spread_run(q, blockIdx.x, blockIdx.y, c0, ix0, iy);
     if (ix0 >= G || iy >= G) return;
     const int tile = blockIdx.y * gridDim.x + blockIdx.x, cidx = tile * 256 + c0;
-    const unsigned o0 = offs[cidx], o1 = offs[cidx + 1], o2 = offs[cidx + 2];
-    if (o1 - o0 > SPREAD_HEAVY || o2 - o1 > SPREAD_HEAVY) return;       // both cells go to k_adj_spread_heavy (k_spread_heavy_list lists partners)
     const int R = d.discR, ks = iy < G / 2 ? iy : iy - G, kf0 = ix0 < G / 2 ? ix0 : ix0 - G;
-    // a cell without taps outside the sampled disc is not written: nobody reads it (see disc_live)
-    const bool st0 = o1 > o0 || kf0 * kf0 + ks * ks <= R * R, st1 = o2 > o1 || (kf0 + 1) * (kf0 + 1) + ks * ks <= R * R;
-    if (!st0 && !st1) return;
-    const unsigned t0 = poffs[tile * 128 + q], t1 = poffs[tile * 128 + q + 1];
-    int ei[8]; float2 ew[8];                                             // entries past the end of the list: (sample 0, weights 0)
+    bool st[SP_NC], any = false;
+    {
+        unsigned o[SP_NC + 1];
 #pragma unroll
-    for (int u = 0; u < 8; ++u) { const bool in = t0 + u < t1; ei[u] = in ? __ldg(&pidx[t0 + u]) : 0; ew[u] = in ? __ldg(&pw[t0 + u]) : make_float2(0.f, 0.f); }
+        for (int c = 0; c <= SP_NC; ++c) o[c] = offs[cidx + c];
+#pragma unroll
+        for (int c = 0; c < SP_NC; ++c) {
+            if (o[c + 1] - o[c] > SPREAD_HEAVY) return;              // the whole run goes to k_adj_spread_heavy (k_spread_heavy_list lists run mates)
+            // a cell without taps outside the sampled disc is not written: nobody reads it (see disc_live)
+            st[c] = o[c + 1] > o[c] || (kf0 + c) * (kf0 + c) + ks * ks <= R * R;
+            any = any || st[c];
+        }
+    }
+    if (!any) return;
+    const unsigned t0 = poffs[tile * SP_RUNS + q], t1 = poffs[tile * SP_RUNS + q + 1];
+    int ei[SP_NR]; SpW ew[SP_NR];                                        // entries past the end of the list: (sample 0, weights 0)
+#pragma unroll
+    for (int u = 0; u < SP_NR; ++u) {
+        const bool in = t0 + u < t1;
+        ei[u] = in ? __ldg(&pidx[t0 + u]) : 0;
+        if (in) ew[u] = spw_load(&pw[t0 + u]);
+        else {
+#pragma unroll
+            for (int c = 0; c < SP_NC; ++c) ew[u].w[c] = 0.f;
+        }
+    }
     const size_t gstride = (size_t)d.na * d.nd * 2, gg2 = (size_t)G * G * 2;
-    float4 *out0 = reinterpret_cast<float4 *>(grid) + (((size_t)iy) * G + (ix0 >> 1)) * 2 + hp;            // ix0 even: first parity block
-    float4 *out1 = out0 + (size_t)(G >> 1) * 2;                                                            // ix0 + 1: the odd block, same position
+    // cell c of the run: parity block (c & 1), position (ix0 >> 1) + (c >> 1)
+    float4 *out = reinterpret_cast<float4 *>(grid) + (((size_t)iy) * G + (ix0 >> 1)) * 2 + hp;
 #pragma unroll 1
     for (int g0 = 0; g0 < ng; g0 += GPT) {
-        float4 a0[GPT], a1[GPT];
+        float4 acc[SP_NC][GPT];
         size_t qoff[GPT];                                               // groups past the end re-read group g0 and are dropped at the store
 #pragma unroll
-        for (int k = 0; k < GPT; ++k) { a0[k] = a1[k] = make_float4(0.f, 0.f, 0.f, 0.f); qoff[k] = g0 + k < ng ? k * gstride : 0; }
+        for (int k = 0; k < GPT; ++k) {
+            qoff[k] = g0 + k < ng ? k * gstride : 0;
+#pragma unroll
+            for (int c = 0; c < SP_NC; ++c) acc[c][k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
         const float4 *cg = reinterpret_cast<const float4 *>(cpol) + (size_t)g0 * gstride + hp;
         if (t1 > t0) {
 #pragma unroll
-            for (int u = 0; u < 4; ++u) pair_tap<GPT>(cg, qoff, ei[u], ew[u], a0, a1);
+            for (int u = 0; u < SP_NR / 2; ++u) run_tap<GPT>(cg, qoff, ei[u], ew[u], acc);
         }
-        if (t1 > t0 + 4) {
+        if (t1 > t0 + SP_NR / 2) {
 #pragma unroll
-            for (int u = 4; u < 8; ++u) pair_tap<GPT>(cg, qoff, ei[u], ew[u], a0, a1);
+            for (int u = SP_NR / 2; u < SP_NR; ++u) run_tap<GPT>(cg, qoff, ei[u], ew[u], acc);
         }
-        for (unsigned t = t0 + 8; t < t1; ++t) pair_tap<GPT>(cg, qoff, __ldg(&pidx[t]), __ldg(&pw[t]), a0, a1);
+        for (unsigned t = t0 + SP_NR; t < t1; ++t) run_tap<GPT>(cg, qoff, __ldg(&pidx[t]), spw_load(&pw[t]), acc);
 #pragma unroll
         for (int k = 0; k < GPT; ++k)
             if (g0 + k < ng) {
-                if (st0) out0[(size_t)(g0 + k) * gg2] = a0[k];
-                if (st1) out1[(size_t)(g0 + k) * gg2] = a1[k];
+#pragma unroll
+                for (int c = 0; c < SP_NC; ++c)
+                    if (st[c]) out[(size_t)(g0 + k) * gg2 + ((size_t)(c & 1) * (G >> 1) + (c >> 1)) * 2] = acc[c][k];
             }
     }
 }
@@ -514,11 +557,12 @@ void launch_spread_count(const DevPlan &d, int *counts, cudaStream_t st) {
 void launch_spread_fill(const DevPlan &d, cudaStream_t st) {
     k_spread_fill<<<dim3((d.G + 31) / 32, (d.G + 7) / 8), 256, 0, st>>>(d, d.tile_rng, d.tile_nr, d.tap_offs, const_cast<int2 *>(d.taps));
 }
+int spread_run_cells() { return SP_NC; }
 void launch_pair_count(const DevPlan &d, unsigned *counts, cudaStream_t st) {
-    k_pair_count<<<dim3((d.G + 31) / 32, (d.G + 7) / 8), 128, 0, st>>>(d, counts);
+    k_run_count<<<dim3((d.G + 31) / 32, (d.G + 7) / 8), SP_RUNS, 0, st>>>(d, counts);
 }
-void launch_pair_fill(const DevPlan &d, int *pidx, float2 *pw, cudaStream_t st) {
-    k_pair_fill<<<dim3((d.G + 31) / 32, (d.G + 7) / 8), 128, 0, st>>>(d, d.pair_offs, pidx, pw);
+void launch_pair_fill(const DevPlan &d, int *pidx, void *pw, cudaStream_t st) {
+    k_run_fill<<<dim3((d.G + 31) / 32, (d.G + 7) / 8), SP_RUNS, 0, st>>>(d, d.pair_offs, pidx, static_cast<SpW *>(pw));
 }
 void launch_spread_heavy_list(const DevPlan &d, unsigned ncell, unsigned *list, unsigned *count, cudaStream_t st) {
     k_spread_heavy_list<<<(ncell + 255) / 256, 256, 0, st>>>(d, d.tap_offs, ncell, list, count);
@@ -542,8 +586,9 @@ void launch_adj_spread(const DevPlan &d, const float2 *cpol, int ng, float2 *gri
     }
     const dim3 bl(512), gr((d.G + 31) / 32, (d.G + 7) / 8, 1);     // the group blocks are looped inside the kernel
     if (d.pair_offs && !env_is("TC_SPREAD", "plain")) {
-        if (ng >= 2) k_adj_spread_pairs<2><<<gr, 256, 0, st>>>(d, d.tap_offs, d.pair_offs, d.pair_idx, d.pair_w, cpol, ng, grid);
-        else k_adj_spread_pairs<1><<<gr, 256, 0, st>>>(d, d.tap_offs, d.pair_offs, d.pair_idx, d.pair_w, cpol, ng, grid);
+        const SpW *pw = static_cast<const SpW *>(d.pair_w);
+        if (ng >= 2) k_adj_spread_runs<2><<<gr, 2 * SP_RUNS, 0, st>>>(d, d.tap_offs, d.pair_offs, d.pair_idx, pw, cpol, ng, grid);
+        else k_adj_spread_runs<1><<<gr, 2 * SP_RUNS, 0, st>>>(d, d.tap_offs, d.pair_offs, d.pair_idx, pw, cpol, ng, grid);
         TC_COUNT_LAUNCH();
         if (hs != st) cudaStreamWaitEvent(st, d.ev_join, 0);
         return;

@@ -45,7 +45,7 @@ struct tc_plan {
     int2 *taps = nullptr;
     unsigned *heavy = nullptr;
     long long n_taps = 0;
-    unsigned *pair_offs = nullptr; int *pair_idx = nullptr; float2 *pair_w = nullptr;      // lists of the cell pairs
+    unsigned *pair_offs = nullptr; int *pair_idx = nullptr; void *pair_w = nullptr;      // lists of the cell runs
     int *gt_tiles = nullptr; unsigned *gt_start = nullptr; int4 *gt_samples = nullptr;   // tile-binned gather tables
     bool gather_tiles = true;     // F3 as k_fwd_gather_tiles + k_fwd_radial (default) or as the fused ray-by-ray k_fwd_gather (TC_GATHER=ray)
     // scratch
@@ -273,7 +273,7 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
         d.tap_offs = p->tap_offs; d.taps = p->taps;
         launch_spread_fill(d, nullptr);
         {   // cells with long lists: at most the disc of radius ~ 36 na / (2 pi SPREAD_HEAVY) cells; size the list for all cells with > SPREAD_HEAVY taps
-            const size_t cap = std::min<size_t>(nc, 2 * ((size_t)total / SPREAD_HEAVY + 1));      // long lists and their pair partners
+            const size_t cap = std::min<size_t>(nc, (size_t)spread_run_cells() * ((size_t)total / SPREAD_HEAVY + 1));      // long lists and the cells of their runs
             unsigned *cnt = nullptr;
             e = cudaMalloc((void **)&p->heavy, cap * sizeof(unsigned));
             if (e == cudaSuccess) e = cudaMalloc((void **)&cnt, sizeof(unsigned));
@@ -290,7 +290,7 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
             if (e != cudaSuccess) { tc_plan_destroy(p); return fail(TC_ECUDA, std::string("spread heavy list: ") + cudaGetErrorString(e)); }
         }
         {   // lists of the cell pairs (k_adj_spread_pairs): count, exclusive scan, fill
-            const size_t np = (size_t)nt * 128;
+            const size_t np = (size_t)nt * (256 / spread_run_cells());
             unsigned *pc = nullptr; void *tmp2 = nullptr; size_t tb2 = 0; unsigned ptotal = 0;
             d.pair_offs = nullptr; d.pair_idx = nullptr; d.pair_w = nullptr;
             e = cudaMalloc((void **)&pc, (np + 1) * sizeof(unsigned));
@@ -305,7 +305,7 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
             if (e == cudaSuccess) e = cudaMemcpy(&ptotal, p->pair_offs + np, sizeof(unsigned), cudaMemcpyDeviceToHost);
             cudaFree(pc); cudaFree(tmp2);
             if (e == cudaSuccess) e = cudaMalloc((void **)&p->pair_idx, (size_t)std::max(ptotal, 1u) * sizeof(int));
-            if (e == cudaSuccess) e = cudaMalloc((void **)&p->pair_w, (size_t)std::max(ptotal, 1u) * sizeof(float2));
+            if (e == cudaSuccess) e = cudaMalloc(&p->pair_w, (size_t)std::max(ptotal, 1u) * sizeof(float) * spread_run_cells());
             if (e != cudaSuccess) { tc_plan_destroy(p); return fail(e == cudaErrorMemoryAllocation ? TC_ENOMEM : TC_ECUDA, std::string("spread pair lists: ") + cudaGetErrorString(e)); }
             d.pair_offs = p->pair_offs;
             launch_pair_fill(d, p->pair_idx, p->pair_w, nullptr);
