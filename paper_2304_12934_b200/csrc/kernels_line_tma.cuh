@@ -118,7 +118,7 @@ static bool launch_fwd_cols_tma_n(const DevPlan &d, const float2 *rowbuf, int ng
     tc_encode_tiled_fn enc = tensor_map_encoder();
     if (!enc) return false;
     using Cfg = typename LtSize<N, 2>::Cfg;
-    static LtMapCache c;
+    static thread_local LtMapCache c;          // per host thread: plans may be used from different threads (one plan, one thread at a time)
     if (c.ptr != rowbuf || c.ng != ng) {
         const cuuint64_t dims[3] = {8, (cuuint64_t)d.G, (cuuint64_t)d.n * ng};
         const cuuint64_t strides[2] = {32, (cuuint64_t)d.G * 32};
@@ -244,7 +244,7 @@ static bool launch_adj_rows_tma_n(const DevPlan &d, const float2 *rowbuf, int S,
     tc_encode_tiled_fn enc = tensor_map_encoder();
     if (!enc) return false;
     using L = LtSize<N, 2>;
-    static LtMapCache c;
+    static thread_local LtMapCache c;          // per host thread: plans may be used from different threads (one plan, one thread at a time)
     if (c.ptr != rowbuf || c.ng != ng) {
         const cuuint64_t n = d.n;
         const cuuint64_t dims[4] = {8, n, 2, n * ng};

@@ -336,6 +336,9 @@ __global__ void __launch_bounds__(256) k_adj_spread_heavy(DevPlan d, const unsig
 // form.  Lists are plan-time data as before; the first SP_NR entries stay in registers across the groups of the slab.
 constexpr int SP_NR = SP_NC == 2 ? 8 : 6;                 // list entries kept in registers
 constexpr int SP_RUNS = 256 / SP_NC;                      // runs per 32 x 8 tile
+#ifndef SP_LB
+#define SP_LB (SP_NC == 2 ? 3 : 4)                        // CTAs per SM the main kernel is compiled for
+#endif
 struct SpW { float w[SP_NC]; };
 
 template <class F>
@@ -419,7 +422,7 @@ __device__ __forceinline__ SpW spw_load(const SpW *p) {
 }
 
 template <int GPT>
-__global__ void __launch_bounds__(2 * SP_RUNS, SP_NC == 2 ? 3 : 4) k_adj_spread_runs(DevPlan d, const unsigned *__restrict__ offs, const unsigned *__restrict__ poffs,
+__global__ void __launch_bounds__(2 * SP_RUNS, SP_LB) k_adj_spread_runs(DevPlan d, const unsigned *__restrict__ offs, const unsigned *__restrict__ poffs,
                                                             const int *__restrict__ pidx, const SpW *__restrict__ pw,
                                                             const float2 *__restrict__ cpol, int ng, float2 *__restrict__ grid) {
     const int q = threadIdx.x >> 1, hp = threadIdx.x & 1, G = d.G;
