@@ -381,6 +381,31 @@ def test_full_size_config3_and_config5_geometry_sampled(tc):
         assert _adj_mismatch(vol, y, s, b) < TOL_ADJ
 
 
+def test_tma_line_kernels_ragged_groups_and_unaligned_input(tc):
+    # The TMA-fed line kernels (n = 1024 here, the same templates as 2048) with a ragged last group (11 slices: 8 + 3, so the float
+    # rows of absent slices are not copied) and with input arrays whose base is not 16-byte aligned (bulk copies need it: the library
+    # must fall back to the plain kernels, same result).  One slice against the oracle, adjoint identity, aligned vs unaligned equal.
+    import torch
+    from paper_2304_12934_b200 import inputs
+    from oracle import nufft
+    S, N, Na, centre = 11, 1024, 24, 515.25
+    ang = inputs.angles_uniform(Na); a64 = ang.astype(np.float64)
+    vol = inputs.volume_porous(S, N, 77)
+    y = np.random.default_rng(78).standard_normal((S, Na, N)).astype(np.float32)
+    plan = tc.Plan(N, N, ang, centre)
+    s = _np(plan.radon(_cuda(vol))); b = _np(plan.backproject(_cuda(y)))
+    assert rel_l2(s[9], nufft.radon_nufft(vol[9], a64, N, centre)) < TOL_NUFFT            # a slice of the ragged group
+    assert rel_l2(b[10], nufft.backproject_nufft(y[10], a64, N, centre)) < TOL_NUFFT
+    assert _adj_mismatch(vol, y, s, b) < TOL_ADJ
+    vbuf = torch.empty(vol.size + 1, dtype=torch.float32, device="cuda"); ybuf = torch.empty(y.size + 1, dtype=torch.float32, device="cuda")
+    vu = vbuf[1:].view(S, N, N); yu = ybuf[1:].view(S, Na, N)                           # base address = 4 (mod 16)
+    vu.copy_(torch.from_numpy(vol)); yu.copy_(torch.from_numpy(y))
+    assert vu.data_ptr() % 16 == 4
+    s2 = _np(plan.radon(vu)); b2 = _np(plan.backproject(yu))
+    plan.close()
+    assert rel_l2(s2, s) < 1e-6 and rel_l2(b2, b) < 1e-6
+
+
 def test_second_workload_shape_2448_bins(tc):
     # the shape of the paper's third data set (202 projections x 2448 columns, Table 1) on a 2560^2 image:
     # n_det = 2448 = 2^4 3^2 17 runs the radix-3 and radix-17 passes of the radial FFT, n_det != n puts 2.09 fine-grid cells between
