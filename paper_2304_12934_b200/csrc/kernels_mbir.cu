@@ -7,7 +7,7 @@
 
 namespace tc {
 
-constexpr int RED_BLOCKS = 1184;     // 148 SMs x 8
+constexpr int RED_BLOCKS = 1184;     // 148 SMs x 8 (<= 2048: the partial-sum area acc[16 ..] holds two sets of 2048)
 constexpr int RED_THREADS = 256;
 
 __device__ __forceinline__ void block_reduce_to(double v, double *partials) {
@@ -35,8 +35,9 @@ __global__ void k_final_reduce(const double *partials, int nb, double *acc, int 
     if (threadIdx.x == 0) acc[slot] += scale * sh[0];
 }
 
-static void final_reduce(double *acc, int slot, double scale, cudaStream_t st) {
-    k_final_reduce<<<1, RED_THREADS, 0, st>>>(acc + 16, RED_BLOCKS, acc, slot, scale);
+// scratch = which half of the partial-sum area (two reductions may run on two streams at once)
+static void final_reduce(double *acc, int slot, double scale, cudaStream_t st, int scratch = 0) {
+    k_final_reduce<<<1, RED_THREADS, 0, st>>>(acc + 16 + scratch * 2048, RED_BLOCKS, acc, slot, scale);
     TC_COUNT_LAUNCH();
 }
 
@@ -399,8 +400,9 @@ void launch_step(const float *x, const float *xm, float beta, const float *g, fl
 }
 void launch_candidate_sino(const float *A0, const float *A1, const float *Ag, const float *b, float beta, float alpha, float *Az, double *acc,
                            size_t n, cudaStream_t st) {
-    k_candidate_sino<<<RED_BLOCKS, RED_THREADS, 0, st>>>(A0, A1, Ag, b, beta, alpha, Az, acc + 16, n); TC_COUNT_LAUNCH();
-    final_reduce(acc, 0, 0.5, st);
+    // second half of the partial-sum area: this reduction may run beside the prior's (launch_prior) on another stream
+    k_candidate_sino<<<RED_BLOCKS, RED_THREADS, 0, st>>>(A0, A1, Ag, b, beta, alpha, Az, acc + 16 + 2048, n); TC_COUNT_LAUNCH();
+    final_reduce(acc, 0, 0.5, st, 1);
 }
 void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, int n, cudaStream_t st, int S_own) {
     if (S_own < 0) S_own = S;

@@ -56,6 +56,7 @@ struct tc_plan {
     float *stage_in[2] = {nullptr, nullptr}, *stage_out[2] = {nullptr, nullptr};
     size_t stage_in_elems = 0, stage_out_elems = 0;
     cudaStream_t s_h2d = nullptr, s_comp = nullptr, s_d2h = nullptr;
+    cudaStream_t s_aux = nullptr; cudaEvent_t ev_aux[2] = {nullptr, nullptr};   // MBIR: the data term of the objective beside the prior term
     tc_sched_stats stats{};
     // per-stage CUDA-event timing (tc_profile)
     bool prof = false, prof_open = false;
@@ -424,6 +425,8 @@ extern "C" tc_status tc_plan_destroy(tc_plan *p) {
     if (p->d.ev_join) cudaEventDestroy(p->d.ev_join);
     for (auto &r : p->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto &e : p->prof_pool) cudaEventDestroy(e);
+    if (p->s_aux) cudaStreamDestroy(p->s_aux);
+    for (auto &ev : p->ev_aux) if (ev) cudaEventDestroy(ev);
     if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
     if (p->s_comp) cudaStreamDestroy(p->s_comp);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);

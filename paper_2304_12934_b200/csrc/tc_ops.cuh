@@ -279,6 +279,10 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
     const size_t nv = (size_t)S * vps, ns = (size_t)S * sps, nvx = (size_t)Sx * vps;
     *retry_streamed = false;
     int slab; TCS(ensure_scratch(p, S, &slab, 16));           // at most 16 groups of FFT scratch: the state below needs the memory
+    if (!p->s_aux) {
+        CU(cudaStreamCreateWithFlags(&p->s_aux, cudaStreamNonBlocking));
+        for (auto &ev : p->ev_aux) CU(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    }
     CallMem mem;
     float *vb[4] = {nullptr}, *sb[5] = {nullptr};
     bool ok = true;
@@ -342,13 +346,20 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
         } else {
             launch_update(xe, xme, beta, ge, pd, invL, ge, ze, Sx, d.n, st, lo, S);           // M2 + M3: g, z = y - g / L on the core
         }
+        // M4.  The data term streams five sinograms (HBM-bound), the prior term is a stencil (MUFU / issue-bound): unless ranks have to
+        // exchange halos in between, the first runs on a second stream beside the second.
+        cudaStream_t sd = st;
+        if (!comm && p->s_aux) sd = p->s_aux;
         if (pd.nonneg) {                                                  // projected candidate: z is not linear in g, so A z itself
             slabbed(forward_slab, z, vps, r, sps);
-            launch_candidate_sino(r, nullptr, nullptr, b, 0.f, 0.f, Az, p->acc, ns, st);      // M4: Az = A z
+            if (sd != st) { CU(cudaEventRecord(p->ev_aux[0], st)); CU(cudaStreamWaitEvent(sd, p->ev_aux[0], 0)); }
+            launch_candidate_sino(r, nullptr, nullptr, b, 0.f, 0.f, Az, p->acc, ns, sd);      // M4: Az = A z
         } else {
             if (!pr->mm_step) slabbed(forward_slab, gv, vps, r, sps);     // A g
-            launch_candidate_sino(Ax, Axm, r, b, beta, alpha, Az, p->acc, ns, st);            // M4: Az = A y - alpha A g
+            if (sd != st) { CU(cudaEventRecord(p->ev_aux[0], st)); CU(cudaStreamWaitEvent(sd, p->ev_aux[0], 0)); }
+            launch_candidate_sino(Ax, Axm, r, b, beta, alpha, Az, p->acc, ns, sd);            // M4: Az = A y - alpha A g
         }
+        if (sd != st) CU(cudaEventRecord(p->ev_aux[1], sd));
         if (comm) {                                                       // the candidate's boundary slices go to the neighbours' halos
             if (lo) CU(cudaMemcpyAsync(comm->send_down, z, vps * sizeof(float), cudaMemcpyDeviceToDevice, st));
             if (hi) CU(cudaMemcpyAsync(comm->send_up, z + (size_t)(S - 1) * vps, vps * sizeof(float), cudaMemcpyDeviceToDevice, st));
@@ -358,6 +369,7 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
             if (hi) CU(cudaMemcpyAsync(ze + (size_t)(Sx - 1) * vps, comm->recv_up, vps * sizeof(float), cudaMemcpyDeviceToDevice, st));
         }
         launch_prior(z, pd, nullptr, p->acc, S + hi, d.n, st, S);         // pairs are owned by their lower slice: the core's, up to the upper halo
+        if (sd != st) CU(cudaStreamWaitEvent(st, p->ev_aux[1], 0));
         if (pr->grad_restart) launch_dot_gzx(gv, z, x, nv, p->acc, 3, st);
         CU(cudaMemcpyAsync(h, p->acc, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
