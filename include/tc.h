@@ -134,6 +134,15 @@ tc_status tc_power_iteration(tc_plan *plan, int iters, double *lambda_hat);
  * *value (HOST, nullable) = H(volume); device or host pointers for volume/grad. */
 tc_status tc_prior_eval(const float *volume, int n_slices, int n, const tc_prior *prior, float *grad, double *value);
 
+/* Stage hooks for the per-stage unit tests: ONE complex plane through ONE stage of the NUFFT, HOST arrays in natural order
+ * (complex = interleaved float pairs).  fine_grid: F1 + F2 of eq. (8) read backwards: slices re, im (im nullable) ->
+ * Ghat[k_y][k_x], G x G, G = 2 n, FFT order, of the plane re + i im (deapodised, zero-padded, 2-D FFT); gather: F3, eq. (7) reversed
+ * (P:L83): Ghat -> c[a][m mod n_det] (before the centre phase; the Nyquist mode stays 0); spread: B2, eq. (7): c -> Ghat.
+ * Cells of Ghat farther than n + kb_width - 1 from the origin are never touched by the method and come back as 0. */
+tc_status tc_stage_fine_grid(tc_plan *plan, const float *re, const float *im, float *grid_out);
+tc_status tc_stage_gather(tc_plan *plan, const float *grid_in, float *cpol_out);
+tc_status tc_stage_spread(tc_plan *plan, const float *cpol_in, float *grid_out);
+
 /* One-shot form with exactly the problem statement's shape = create plan, tc_radon, destroy. */
 tc_status tc_radon1(const float *volume, int n_slices, int n, const float *angles, int n_angles, int n_det,
                     float center, float *sinogram);

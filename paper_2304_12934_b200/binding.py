@@ -57,6 +57,9 @@ lib.tc_fbp.argtypes = [_vp, _vp, _ci, _ci, _vp, _vp]
 lib.tc_mbir.argtypes = [_vp, _vp, _ci, ctypes.POINTER(tc_prior), _ci, _vp, ctypes.POINTER(tc_iter_log), _vp]
 lib.tc_mbir_sharded.argtypes = [_vp, _vp, _ci, ctypes.POINTER(tc_prior), _ci, _vp, ctypes.POINTER(tc_iter_log), ctypes.POINTER(tc_comm), _vp]
 lib.tc_power_iteration.argtypes = [_vp, _ci, ctypes.POINTER(ctypes.c_double)]
+lib.tc_stage_fine_grid.argtypes = [_vp, _vp, _vp, _vp]
+lib.tc_stage_gather.argtypes = [_vp, _vp, _vp]
+lib.tc_stage_spread.argtypes = [_vp, _vp, _vp]
 lib.tc_prior_eval.argtypes = [_vp, _ci, _ci, ctypes.POINTER(tc_prior), _vp, ctypes.POINTER(ctypes.c_double)]
 lib.tc_radon1.argtypes = [_vp, _ci, _ci, ctypes.POINTER(ctypes.c_float), _ci, _ci, ctypes.c_float, _vp]
 lib.tc_launch_count.argtypes = [_ci]
@@ -207,6 +210,26 @@ class Plan:
         ms = (ctypes.c_double * 8)(); cnt = (ctypes.c_longlong * 8)()
         _check(lib.tc_profile_read(self._h, ms, cnt))
         return {k: (ms[i], cnt[i]) for i, k in enumerate(self.STAGES)}
+
+    # stage hooks (per-stage unit tests): numpy host arrays, complex64 in natural order
+    def stage_fine_grid(self, re, im=None):
+        re = np.ascontiguousarray(re, dtype=np.float32)
+        im = None if im is None else np.ascontiguousarray(im, dtype=np.float32)
+        out = np.empty((2 * self.n, 2 * self.n), dtype=np.complex64)
+        _check(lib.tc_stage_fine_grid(self._h, re.ctypes.data, None if im is None else im.ctypes.data, out.ctypes.data))
+        return out
+
+    def stage_gather(self, grid):
+        grid = np.ascontiguousarray(grid, dtype=np.complex64)
+        out = np.empty((self.n_angles, self.n_det), dtype=np.complex64)
+        _check(lib.tc_stage_gather(self._h, grid.ctypes.data, out.ctypes.data))
+        return out
+
+    def stage_spread(self, cpol):
+        cpol = np.ascontiguousarray(cpol, dtype=np.complex64)
+        out = np.empty((2 * self.n, 2 * self.n), dtype=np.complex64)
+        _check(lib.tc_stage_spread(self._h, cpol.ctypes.data, out.ctypes.data))
+        return out
 
     def sched_stats(self):
         s = tc_sched_stats()

@@ -37,7 +37,7 @@ def build(force=False, verbose=False):
             sys.stderr.write(r.stdout + r.stderr)
         if r.returncode:
             raise RuntimeError("nvcc failed on " + src)
-    r = subprocess.run([NVCC, "-shared", "-o", LIB, *[o for _, o, _ in res], "-lcudart"], capture_output=True, text=True)
+    r = subprocess.run([NVCC, "-shared", "-o", LIB, *[o for _, o, _ in res], "-lcudart", "-ldl"], capture_output=True, text=True)
     if r.returncode:
         sys.stderr.write(r.stdout + r.stderr)
         raise RuntimeError("link failed")

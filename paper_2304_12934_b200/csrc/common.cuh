@@ -132,6 +132,10 @@ void launch_scale(float *v, float a, size_t n, cudaStream_t st);
 // sino[s][a][u] = -log(max((proj[a][s][u] - dark[s][u]) / (flat[s][u] - dark[s][u]), floor))   (Beer-Lambert + reorder)
 void launch_preprocess(const float *proj, const float *flat, const float *dark, int na, int S, int nd, float floor_, float *sino, cudaStream_t st);
 
+// test hooks (tc_stage_*): one complex plane of group 0 in natural order <-> the internal layouts
+void launch_grid_plane(float2 *grid, float2 *nat, int G, int pl, bool put, cudaStream_t st);
+void launch_cpol_plane(float2 *cpol, float2 *nat, size_t n, int pl, bool put, cudaStream_t st);
+
 long long &launch_counter();
 
 }  // namespace tc

@@ -176,6 +176,28 @@ __global__ void TC_LB2 k_adj_rows(DevPlan d, const float2 *__restrict__ rowbuf, 
     }
 }
 
+// ---- test hooks: one complex plane in / out of the internal layouts (tc_stage_*, per-stage unit tests) ----------------------------
+// nat[y][x] (row y <-> k_y, natural order) <-> plane `pl` of group 0 of the fine grid, grid[x][y & 1][y >> 1][P]
+__global__ void k_grid_plane(float2 *grid, float2 *nat, int G, int pl, int put) {
+    const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    if (i >= (size_t)G * G) return;
+    const int y = (int)(i / G), x = (int)(i % G);
+    float2 *cell = grid + (((size_t)x * G) + (size_t)(y & 1) * (G >> 1) + (y >> 1)) * 4 + pl;
+    if (put) *cell = nat[i]; else nat[i] = *cell;
+}
+// nat[a][k] (k = m mod nd) <-> plane `pl` of group 0 of the polar coefficients, cpol[a][k][P]
+__global__ void k_cpol_plane(float2 *cpol, float2 *nat, size_t n, int pl, int put) {
+    const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    if (put) cpol[i * 4 + pl] = nat[i]; else nat[i] = cpol[i * 4 + pl];
+}
+void launch_grid_plane(float2 *grid, float2 *nat, int G, int pl, bool put, cudaStream_t st) {
+    k_grid_plane<<<(unsigned)(((size_t)G * G + 255) / 256), 256, 0, st>>>(grid, nat, G, pl, put ? 1 : 0);
+}
+void launch_cpol_plane(float2 *cpol, float2 *nat, size_t n, int pl, bool put, cudaStream_t st) {
+    k_cpol_plane<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(cpol, nat, n, pl, put ? 1 : 0);
+}
+
 #include "kernels_polar.cuh"
 #include "kernels_gather_tiles.cuh"
 #include "kernels_line_tma.cuh"

@@ -9,6 +9,7 @@
 #include <algorithm>
 #include "../../include/tc.h"
 #include "common.cuh"
+#include <nvtx3/nvToolsExt.h>      // header-only NVTX: named ranges for Nsight timelines (stages, MBIR iterations); no-ops without a tool
 #include <cub/device/device_scan.cuh>
 #include <cub/device/device_radix_sort.cuh>
 
@@ -89,7 +90,9 @@ static void prof_stage(tc_plan *p, int stage, cudaStream_t st, bool begin) {
         p->prof_open = false;
     }
 }
-#define STAGE(id, call) do { prof_stage(p, id, st, true); call; prof_stage(p, id, st, false); } while (0)
+static const char *const STAGE_NAMES[TC_N_STAGES] = {"F1 fwd_rows", "F2 fwd_cols", "F3 fwd_gather", "B1 adj_radial", "B2 adj_spread", "B3 adj_cols", "B3+B4 adj_rows", "F4 fwd_radial"};
+struct NvtxRange { explicit NvtxRange(const char *name) { nvtxRangePushA(name); } ~NvtxRange() { nvtxRangePop(); } };
+#define STAGE(id, call) do { NvtxRange nv_(STAGE_NAMES[id]); prof_stage(p, id, st, true); call; prof_stage(p, id, st, false); } while (0)
 
 // ---- host-side mathematics of the plan (float64) ---------------------------------------------------
 static double bessel_i0(double x) {          // I0(x) = sum_k (x^2/4)^k / (k!)^2

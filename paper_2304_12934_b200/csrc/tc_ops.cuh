@@ -187,6 +187,66 @@ extern "C" tc_status tc_preprocess(const float *proj, const float *flat, const f
     return TC_OK;
 }
 
+// ---- stage test hooks (unit tier): one complex plane through ONE stage, host arrays in natural order ----------
+// F1 + F2: slices re / im (im nullable) -> the fine grid Ghat[k_y][k_x] of the plane re + i im (cells outside the sampled disc: 0)
+extern "C" tc_status tc_stage_fine_grid(tc_plan *p, const float *re, const float *im, float *grid_out) {
+    if (!p || !re || !grid_out) return fail(TC_EINVAL, "null argument");
+    const DevPlan &d = p->d;
+    const size_t nv = (size_t)d.n * d.n, ng2 = (size_t)d.G * d.G;
+    int slab; TCS(ensure_scratch(p, 8, &slab));
+    CallMem mem;
+    float *vol = nullptr; float2 *nat = nullptr;
+    CU(mem.alloc(&vol, 8 * nv)); CU(mem.alloc(&nat, ng2));
+    CU(cudaMemset(vol, 0, 8 * nv * sizeof(float)));
+    CU(cudaMemcpy(vol, re, nv * sizeof(float), cudaMemcpyHostToDevice));
+    if (im) CU(cudaMemcpy(vol + nv, im, nv * sizeof(float), cudaMemcpyHostToDevice));
+    CU(cudaMemset(p->grid, 0, ng2 * P * sizeof(float2)));
+    launch_fwd_rows(d, vol, 8, 1, p->rowbuf, nullptr);
+    launch_fwd_cols(d, p->rowbuf, 1, p->grid, nullptr);
+    launch_grid_plane(p->grid, nat, d.G, 0, false, nullptr);
+    TCS(check_launch());
+    CU(cudaMemcpy(grid_out, nat, ng2 * sizeof(float2), cudaMemcpyDeviceToHost));
+    return TC_OK;
+}
+// F3: fine grid Ghat[k_y][k_x] -> polar coefficients c[a][m mod nd] (before the centre phase; the Nyquist mode is not computed: 0)
+extern "C" tc_status tc_stage_gather(tc_plan *p, const float *grid_in, float *cpol_out) {
+    if (!p || !grid_in || !cpol_out) return fail(TC_EINVAL, "null argument");
+    const DevPlan &d = p->d;
+    const size_t ng2 = (size_t)d.G * d.G, ns = (size_t)d.na * d.nd;
+    int slab; TCS(ensure_scratch(p, 8, &slab));
+    CallMem mem;
+    float2 *nat = nullptr, *natc = nullptr;
+    CU(mem.alloc(&nat, ng2)); CU(mem.alloc(&natc, ns));
+    CU(cudaMemcpy(nat, grid_in, ng2 * sizeof(float2), cudaMemcpyHostToDevice));
+    CU(cudaMemset(p->grid, 0, ng2 * P * sizeof(float2)));
+    CU(cudaMemset(p->cpol, 0, ns * P * sizeof(float2)));
+    launch_grid_plane(p->grid, nat, d.G, 0, true, nullptr);
+    launch_fwd_gather_tiles(d, p->grid, 1, p->cpol, nullptr);
+    launch_cpol_plane(p->cpol, natc, ns, 0, false, nullptr);
+    TCS(check_launch());
+    CU(cudaMemcpy(cpol_out, natc, ns * sizeof(float2), cudaMemcpyDeviceToHost));
+    return TC_OK;
+}
+// B2: polar coefficients c[a][m mod nd] -> fine grid Ghat[k_y][k_x] (cells outside the sampled disc: 0)
+extern "C" tc_status tc_stage_spread(tc_plan *p, const float *cpol_in, float *grid_out) {
+    if (!p || !cpol_in || !grid_out) return fail(TC_EINVAL, "null argument");
+    const DevPlan &d = p->d;
+    const size_t ng2 = (size_t)d.G * d.G, ns = (size_t)d.na * d.nd;
+    int slab; TCS(ensure_scratch(p, 8, &slab));
+    CallMem mem;
+    float2 *nat = nullptr, *natc = nullptr;
+    CU(mem.alloc(&nat, ng2)); CU(mem.alloc(&natc, ns));
+    CU(cudaMemcpy(natc, cpol_in, ns * sizeof(float2), cudaMemcpyHostToDevice));
+    CU(cudaMemset(p->grid, 0, ng2 * P * sizeof(float2)));
+    CU(cudaMemset(p->cpol, 0, ns * P * sizeof(float2)));
+    launch_cpol_plane(p->cpol, natc, ns, 0, true, nullptr);
+    launch_adj_spread(d, p->cpol, 1, p->grid, nullptr);
+    launch_grid_plane(p->grid, nat, d.G, 0, false, nullptr);
+    TCS(check_launch());
+    CU(cudaMemcpy(grid_out, nat, ng2 * sizeof(float2), cudaMemcpyDeviceToHost));
+    return TC_OK;
+}
+
 // ---- prior test hook ---------------------------------------------------------------------------------
 static tc_status check_prior(const tc_prior *pr) {
     if (!pr) return fail(TC_EINVAL, "null prior");
@@ -320,6 +380,7 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
         for (int s0 = 0; s0 < S; s0 += slab) op(p, in + (size_t)s0 * ips, std::min(slab, S - s0), out + (size_t)s0 * ops, st);
     };
     for (int it = 0; it < iters; ++it) {
+        NvtxRange nv_it("tc_mbir iteration");
         const double tp = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));
         const float beta = (float)((t - 1.0) / tp);
         if (it > 0 && it % AX_REFRESH == 0) {                             // A x, A x- from scratch

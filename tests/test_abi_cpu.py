@@ -17,7 +17,7 @@ def test_library_exports_every_declared_symbol():
     names = set(re.findall(r"\b(tc_[a-z0-9_]+)\s*\(", hdr))
     assert {"tc_plan_create", "tc_plan_destroy", "tc_radon", "tc_backproject", "tc_mbir", "tc_radon1",
             "tc_power_iteration", "tc_prior_eval", "tc_last_error", "tc_launch_count", "tc_last_sched_stats", "tc_fbp",
-            "tc_mbir_sharded", "tc_preprocess", "tc_host_alloc", "tc_host_free"} <= names
+            "tc_mbir_sharded", "tc_preprocess", "tc_host_alloc", "tc_host_free", "tc_stage_fine_grid", "tc_stage_gather", "tc_stage_spread"} <= names
     lib = _lib()
     for n in names:
         assert hasattr(lib, n), n

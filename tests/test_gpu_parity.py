@@ -61,6 +61,39 @@ def test_config1_forward_adjoint_vs_oracle_and_direct(tc):
     assert _adj_mismatch(vol, yr, s2, b2) < TOL_ADJ
 
 
+@pytest.mark.parametrize("N,Nd,Na,W", [(64, 64, 45, 6), (160, 200, 13, 6), (96, 144, 9, 8)])
+def test_stages_one_by_one_vs_oracle(tc, N, Nd, Na, W):
+    # SURVEY section 4, unit tier: each NUFFT stage on its own against the oracle's stage of the same name, one complex plane
+    # (two real slices packed as re + i im, as the library packs them).  F1 + F2 vs numpy's fft2 of the oracle's padded, deapodised
+    # image; F3 vs oracle.gather on the SAME fine grid; B2 vs oracle.spread on the same coefficients.  1e-5 relative L2.
+    from oracle import nufft
+    rng = np.random.default_rng(N + Nd)
+    ang = np.sort(rng.uniform(0, math.pi, Na)).astype(np.float32); a64 = ang.astype(np.float64)
+    G = 2 * N
+    plan = tc.Plan(N, Nd, ang, 0.5 * Nd + 1.25, kb_width=W)
+    f0 = rng.random((N, N)).astype(np.float32); f1 = rng.random((N, N)).astype(np.float32)
+    # cells the method never touches (farther than G/2 + W - 1 from the origin) come back as 0: compare inside the disc
+    k = np.fft.fftfreq(G, 1.0 / G)
+    live = (k[:, None] ** 2 + k[None, :] ** 2) <= (G // 2 + W - 1) ** 2
+    ref = np.fft.fft2(nufft.pad_deapod(f0, G, W) + 1j * nufft.pad_deapod(f1, G, W))
+    got = plan.stage_fine_grid(f0, f1)
+    rel_c = lambda a, b: float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(np.asarray(b).ravel()))      # complex arrays
+    assert rel_c(np.where(live, got, 0), np.where(live, ref, 0)) < 1e-5
+    assert np.all(got[~live] == 0)
+    gh = (rng.standard_normal((G, G)) + 1j * rng.standard_normal((G, G))).astype(np.complex64)
+    modes = np.arange(-(Nd // 2) + 1, Nd // 2)
+    c_ref = nufft.gather(gh.astype(np.complex128), a64, Nd, W)                      # (Na, Nd - 1), modes ascending
+    c_got = plan.stage_gather(gh)
+    assert rel_c(c_got[:, modes % Nd], c_ref) < 1e-5
+    assert np.all(c_got[:, Nd // 2] == 0)                                          # the Nyquist mode is excluded (reading G2)
+    c = np.zeros((Na, Nd), np.complex64)
+    c[:, modes % Nd] = (rng.standard_normal((Na, Nd - 1)) + 1j * rng.standard_normal((Na, Nd - 1))).astype(np.complex64)
+    s_ref = nufft.spread(c[:, modes % Nd].astype(np.complex128), a64, Nd, G, W)
+    s_got = plan.stage_spread(c)
+    plan.close()
+    assert rel_c(s_got, s_ref) < 1e-5
+
+
 def test_config2_forward_adjoint(tc):
     from paper_2304_12934_b200 import inputs
     from oracle import nufft, direct
