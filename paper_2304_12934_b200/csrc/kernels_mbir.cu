@@ -3,6 +3,7 @@
 // Reductions accumulate in float64 and are deterministic: per-block partials, then one block adds them
 // to the accumulator slot.  Accumulator layout: acc[0..15] results, acc[16 .. 16+RED_BLOCKS) scratch.
 #include <cmath>
+#include <algorithm>
 #include "common.cuh"
 
 namespace tc {
@@ -158,7 +159,7 @@ __device__ __forceinline__ float wgt(int dz, int dy, int dx) {
 // through a chunk of slices: at slice s a thread evaluates its 4 in-plane forward pairs and its 9 pairs with slice s + 1,
 // leaves d in shared memory for the partner (the in-plane ones are picked up in the same step, the 9 others in the next
 // step), and the interior threads write g and z.  One warm-up step below the chunk supplies the first slice's incoming pairs.
-constexpr int PM_ZC = 16;        // output slices per chunk
+constexpr int PM_ZC_MIN = 16, PM_ZC_MAX = 64;   // output slices per chunk: chosen per launch (pm_chunk)
 #ifndef PM_TY
 #define PM_TY 12
 #endif
@@ -169,7 +170,7 @@ constexpr int PM_THREADS = (PM_LIVE + 31) / 32 * 32;
 template <bool STEP, bool EXTRAP>
 __global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__restrict__ y, const float *__restrict__ xm, float beta,
                                                                  const float *atr, PriorK pk, float lambda,
-                                                                 float invL, float *g, float *__restrict__ z, int S, int n, int s_first, int n_out) {
+                                                                 float invL, float *g, float *__restrict__ z, int S, int n, int s_first, int n_out, int PM_ZC) {
     __shared__ float val[2][PM_HY][34];
     __shared__ float din[4][PM_HY][34];
     __shared__ float dup[2][9][PM_HY][34];
@@ -266,7 +267,7 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__
 //   sum over pairs of w h'(D)/D (g_m - g_n)^2,  D = y_m - y_n,  y = x + beta (x - x-) formed on load.
 template <bool CURV>
 __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *__restrict__ zv, const float *__restrict__ xm, float beta,
-                                                                  const float *__restrict__ gdir, PriorK pk, double *partials, int S, int n, int S_own) {
+                                                                  const float *__restrict__ gdir, PriorK pk, double *partials, int S, int n, int S_own, int PM_ZC) {
     __shared__ float val[2][PM_HY][34];
     __shared__ float gval[CURV ? 2 : 1][CURV ? PM_HY : 1][CURV ? 34 : 1];
     __shared__ double red[PM_THREADS / 32];
@@ -364,6 +365,13 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *_
 }
 
 // ---- wrappers -------------------------------------------------------------------------------------
+// A chunk starts with one warm-up slice step, so long chunks waste less (128 slices of 2048^2: MBIR iteration 33.5 ms with 16-slice
+// chunks, 32.1 ms with 64); short ones keep small problems spread over the SMs: as long as tiles x chunks fill the machine.
+static int pm_chunk(int n, int S) {
+    const long long tiles = (long long)((n + 31) / 32) * ((n + PM_TY - 1) / PM_TY);
+    const int nch_min = (int)((RED_BLOCKS + tiles - 1) / tiles);
+    return std::max(PM_ZC_MIN, std::min(PM_ZC_MAX, S / std::max(nch_min, 1)));
+}
 static int ew_blocks(size_t n) { size_t b = (n + 255) / 256; return (int)(b < 148 * 16 ? (b ? b : 1) : 148 * 16); }
 // forward-offset order of the march kernels: o = 0..3 in plane (dy, dx) = (0, 1), (1, -1), (1, 0), (1, 1); o = 4..12: dz = 1, (dy, dx) row-major
 static PriorK mk(PriorDev pr) {
@@ -384,14 +392,15 @@ void launch_residual(const float *Ax, const float *Axm, const float *b, float be
 void launch_update(const float *x, const float *xm, float beta, const float *atr, PriorDev pr, float invL, float *g, float *z, int S, int n,
                    cudaStream_t st, int s_first, int n_out) {
     if (n_out < 0) n_out = S - s_first;
+    const int PM_ZC = pm_chunk(n, n_out);
     dim3 gr((n + 31) / 32, (n + PM_TY - 1) / PM_TY, (n_out + PM_ZC - 1) / PM_ZC);
     const PriorK k = mk(pr);
     if (xm) {
-        if (z) k_prior_grad_march<true, true><<<gr, PM_THREADS, 0, st>>>(x, xm, beta, atr, k, pr.lambda, invL, g, z, S, n, s_first, n_out);
-        else   k_prior_grad_march<false, true><<<gr, PM_THREADS, 0, st>>>(x, xm, beta, atr, k, pr.lambda, invL, g, nullptr, S, n, s_first, n_out);
+        if (z) k_prior_grad_march<true, true><<<gr, PM_THREADS, 0, st>>>(x, xm, beta, atr, k, pr.lambda, invL, g, z, S, n, s_first, n_out, PM_ZC);
+        else   k_prior_grad_march<false, true><<<gr, PM_THREADS, 0, st>>>(x, xm, beta, atr, k, pr.lambda, invL, g, nullptr, S, n, s_first, n_out, PM_ZC);
     } else {
-        if (z) k_prior_grad_march<true, false><<<gr, PM_THREADS, 0, st>>>(x, nullptr, 0.f, atr, k, pr.lambda, invL, g, z, S, n, s_first, n_out);
-        else   k_prior_grad_march<false, false><<<gr, PM_THREADS, 0, st>>>(x, nullptr, 0.f, atr, k, pr.lambda, invL, g, nullptr, S, n, s_first, n_out);
+        if (z) k_prior_grad_march<true, false><<<gr, PM_THREADS, 0, st>>>(x, nullptr, 0.f, atr, k, pr.lambda, invL, g, z, S, n, s_first, n_out, PM_ZC);
+        else   k_prior_grad_march<false, false><<<gr, PM_THREADS, 0, st>>>(x, nullptr, 0.f, atr, k, pr.lambda, invL, g, nullptr, S, n, s_first, n_out, PM_ZC);
     }
     TC_COUNT_LAUNCH();
 }
@@ -408,12 +417,12 @@ void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, 
     if (S_own < 0) S_own = S;
     if (grad) { PriorDev p1 = pr; p1.lambda = 1.f; launch_update(z, nullptr, 0.f, nullptr, p1, 0.f, grad, nullptr, S, n, st); }
     if (acc) {
-        k_prior_value_march<false><<<RED_BLOCKS, PM_THREADS, 0, st>>>(z, nullptr, 0.f, nullptr, mk(pr), acc + 16, S, n, S_own); TC_COUNT_LAUNCH();
+        k_prior_value_march<false><<<RED_BLOCKS, PM_THREADS, 0, st>>>(z, nullptr, 0.f, nullptr, mk(pr), acc + 16, S, n, S_own, pm_chunk(n, S_own)); TC_COUNT_LAUNCH();
         final_reduce(acc, 1, 1.0, st);
     }
 }
 void launch_prior_curvature(const float *x, const float *xm, float beta, const float *g, PriorDev pr, double *acc, int slot, int S, int n, cudaStream_t st) {
-    k_prior_value_march<true><<<RED_BLOCKS, PM_THREADS, 0, st>>>(x, xm, beta, g, mk(pr), acc + 16, S, n, S); TC_COUNT_LAUNCH();
+    k_prior_value_march<true><<<RED_BLOCKS, PM_THREADS, 0, st>>>(x, xm, beta, g, mk(pr), acc + 16, S, n, S, pm_chunk(n, S)); TC_COUNT_LAUNCH();
     final_reduce(acc, slot, 1.0, st);
 }
 void launch_sumsq(const float *v, size_t n, double *acc, int slot, cudaStream_t st) {
