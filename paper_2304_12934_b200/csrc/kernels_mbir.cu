@@ -116,7 +116,8 @@ __global__ void k_scale(float *v, float a, size_t n) {
 
 // ---- qGGMRF stencil -----------------------------------------------------------------------------
 // h(D) = u^2 / (c + u^(2-p)), h'(D) = sign(D)/sigma * u (2c + p u^(2-p)) / (c + u^(2-p))^2, u = |D|/sigma.
-struct PriorK { float inv_sigma, c, p, q; int nonneg; unsigned allow; float wscale; };
+struct PriorK { float inv_sigma, c, p, q; int nonneg; unsigned allow; float wscale; float k0, is2; };
+// k0 = q lg2(1 / sigma): u^q = 2^(q lg2|D| + k0), one FFMA instead of two FMUL; is2 = 1 / sigma^2 (folded into the pair weights).
 // q = 2 - p; nonneg: project the candidate on z >= 0; allow: which of the 13 forward offsets belong to the neighbour set (26: all;
 // 10: the 8 in-plane neighbours and the two along z; 6: faces), wscale: renormalises the 1/distance weights to sum 1 over the set
 
@@ -125,32 +126,31 @@ struct PriorK { float inv_sigma, c, p, q; int nonneg; unsigned allow; float wsca
 __device__ __forceinline__ float lg2a(float x) { float r; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float ex2a(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float rcpa(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
-__device__ __forceinline__ float upow(float u, const PriorK &k) { return k.q == 0.f ? 1.f : ex2a(k.q * lg2a(u)); }     // u^q, u >= 0
+__device__ __forceinline__ float upowD(float D, const PriorK &k) { return k.q == 0.f ? 1.f : ex2a(fmaf(k.q, lg2a(fabsf(D)), k.k0)); }   // (|D| / sigma)^q
 
-// h'(D) = D / sigma^2 * (2c + p u^q) / (c + u^q)^2   (= sign(D)/sigma * u (...) / (...)^2 with u = |D|/sigma)
+// The three evaluations below come WITHOUT the factor 1 / sigma^2: the callers multiply by W = w_mn / sigma^2 (one constant per offset class).
+// h'(D) sigma^2 = D (2c + p u^q) / (c + u^q)^2   (h'(D) = sign(D)/sigma * u (...) / (...)^2 with u = |D|/sigma)
 __device__ __forceinline__ float dh(float D, const PriorK &k) {
-    const float uq = upow(fabsf(D) * k.inv_sigma, k);
+    const float uq = upowD(D, k);
     const float r = rcpa(k.c + uq);
-    return (D * r) * (fmaf(k.p, uq, 2.f * k.c) * r) * (k.inv_sigma * k.inv_sigma);
+    return (D * r) * (fmaf(k.p, uq, 2.f * k.c) * r);
 }
-__device__ __forceinline__ float hval(float D, const PriorK &k) {
-    const float u = fabsf(D) * k.inv_sigma;
-    return u * u * rcpa(k.c + upow(u, k));
-}
-// h'(D) / D = (2c + p u^q) / (sigma^2 (c + u^q)^2): the curvature of the quadratic surrogate of h at D (finite at D = 0: 2 / (c sigma^2))
+// h(D) sigma^2 = D^2 / (c + u^q)
+__device__ __forceinline__ float hval(float D, const PriorK &k) { return D * D * rcpa(k.c + upowD(D, k)); }
+// h'(D) / D sigma^2 = (2c + p u^q) / (c + u^q)^2: the curvature of the quadratic surrogate of h at D (finite at D = 0: 2 / c)
 __device__ __forceinline__ float hcurv(float D, const PriorK &k) {
-    const float uq = upow(fabsf(D) * k.inv_sigma, k);
+    const float uq = upowD(D, k);
     const float r = rcpa(k.c + uq);
-    return (fmaf(k.p, uq, 2.f * k.c) * r) * (r * (k.inv_sigma * k.inv_sigma));
+    return (fmaf(k.p, uq, 2.f * k.c) * r) * r;
 }
 
 // w_mn = (1/dist) / (6 + 12/sqrt2 + 8/sqrt3)  (reading G10)
 #define TC_W_FACE 0.05234482976f
 #define TC_W_EDGE 0.03701338413f
 #define TC_W_CORN 0.03022130267f
-__device__ __forceinline__ float wgt(int dz, int dy, int dx) {
+__device__ __forceinline__ float wgt(int dz, int dy, int dx, float is2) {      // w_mn / sigma^2
     const int k = dz * dz + dy * dy + dx * dx;
-    return k == 1 ? TC_W_FACE : (k == 2 ? TC_W_EDGE : TC_W_CORN);
+    return (k == 1 ? TC_W_FACE : (k == 2 ? TC_W_EDGE : TC_W_CORN)) * is2;
 }
 
 // M2 + M3, pair-sharing form.  h' is odd, so the pair {m, n} gives +d to m and -d to n with d = w h'(y_m - y_n): every pair
@@ -219,7 +219,7 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__
 #pragma unroll
                 for (int dx = -1; dx <= 1; ++dx) {
                     if (dy == 0 && dx <= 0) continue;
-                    const float ev = wgt(0, dy, dx) * dh(c_cur - vc[dy * 34 + dx], pk);       // evaluated unconditionally (a NaN halo is selected away)
+                    const float ev = wgt(0, dy, dx, pk.is2) * dh(c_cur - vc[dy * 34 + dx], pk);       // evaluated unconditionally (a NaN halo is selected away)
                     const float dv = (mk >> o & 1) ? ev : 0.f;
                     din[o][hy][hx] = dv; acc += dv; ++o;
                 }
@@ -227,7 +227,7 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_grad_march(const float *__
             for (int dy = -1; dy <= 1; ++dy)
 #pragma unroll
                 for (int dx = -1; dx <= 1; ++dx) {
-                    const float ev = wgt(1, dy, dx) * dh(c_cur - vu[dy * 34 + dx], pk);
+                    const float ev = wgt(1, dy, dx, pk.is2) * dh(c_cur - vu[dy * 34 + dx], pk);
                     const float dv = (mk >> o & 1) ? ev : 0.f;
                     dup[zz & 1][o - 4][hy][hx] = dv; acc += dv; ++o;
                 }
@@ -328,8 +328,8 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *_
                         if (dy == 0 && dx <= 0) continue;
                         {
                             float ev;
-                            if (CURV) { const float dg = g_cur - gc[dy * 34 + dx]; ev = wgt(0, dy, dx) * hcurv(c_cur - vc[dy * 34 + dx], pk) * (dg * dg); }
-                            else ev = wgt(0, dy, dx) * hval(c_cur - vc[dy * 34 + dx], pk);
+                            if (CURV) { const float dg = g_cur - gc[dy * 34 + dx]; ev = wgt(0, dy, dx, pk.is2) * hcurv(c_cur - vc[dy * 34 + dx], pk) * (dg * dg); }
+                            else ev = wgt(0, dy, dx, pk.is2) * hval(c_cur - vc[dy * 34 + dx], pk);
                             acc += (mk >> o & 1) ? ev : 0.f;
                         }
                         ++o;
@@ -340,8 +340,8 @@ __global__ void __launch_bounds__(PM_THREADS) k_prior_value_march(const float *_
                     for (int dx = -1; dx <= 1; ++dx) {
                         {
                             float ev;
-                            if (CURV) { const float dg = g_cur - gu[dy * 34 + dx]; ev = wgt(1, dy, dx) * hcurv(c_cur - vu[dy * 34 + dx], pk) * (dg * dg); }
-                            else ev = wgt(1, dy, dx) * hval(c_cur - vu[dy * 34 + dx], pk);
+                            if (CURV) { const float dg = g_cur - gu[dy * 34 + dx]; ev = wgt(1, dy, dx, pk.is2) * hcurv(c_cur - vu[dy * 34 + dx], pk) * (dg * dg); }
+                            else ev = wgt(1, dy, dx, pk.is2) * hval(c_cur - vu[dy * 34 + dx], pk);
                             acc += (mk >> o & 1) ? ev : 0.f;
                         }
                         ++o;
@@ -376,6 +376,7 @@ static int ew_blocks(size_t n) { size_t b = (n + 255) / 256; return (int)(b < 14
 // forward-offset order of the march kernels: o = 0..3 in plane (dy, dx) = (0, 1), (1, -1), (1, 0), (1, 1); o = 4..12: dz = 1, (dy, dx) row-major
 static PriorK mk(PriorDev pr) {
     PriorK k; k.inv_sigma = 1.f / pr.sigma; k.c = pr.c; k.p = pr.p; k.q = 2.f - pr.p; k.nonneg = pr.nonneg;
+    k.k0 = (float)((2.0 - (double)pr.p) * std::log2(1.0 / (double)pr.sigma)); k.is2 = (float)(1.0 / ((double)pr.sigma * pr.sigma));
     const double s26 = 6.0 + 12.0 / std::sqrt(2.0) + 8.0 / std::sqrt(3.0);
     if (pr.nbr == 10) { k.allow = 0xFu | (1u << 8); k.wscale = (float)(s26 / (6.0 + 4.0 / std::sqrt(2.0))); }       // 8 in plane + 2 along z
     else if (pr.nbr == 6) { k.allow = (1u << 0) | (1u << 2) | (1u << 8); k.wscale = (float)(s26 / 6.0); }              // faces
