@@ -134,6 +134,14 @@ tc_status tc_power_iteration(tc_plan *plan, int iters, double *lambda_hat);
  * *value (HOST, nullable) = H(volume); device or host pointers for volume/grad. */
 tc_status tc_prior_eval(const float *volume, int n_slices, int n, const tc_prior *prior, float *grad, double *value);
 
+/* tc_radon without any allocation, for callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): the FFT scratch is a 16 MiB static device array of the library (held by every GPU that loads it, until exit)
+ * instead of the plan's lazily allocated buffers.  DEVICE pointers only, ordered on cuda_stream; limits: n <= 256 and
+ * n_angles * n_det <= 131072 (TC_EUNSUPPORTED beyond, with the sizes in tc_last_error); any n_slices (groups of 8, one after the
+ * other).  Same result as tc_radon.  All calls on a device share the array, which keeps the last call's contents: calls that
+ * overlap on the GPU (two streams, plans or host threads) race.  The array's address is looked up at tc_plan_create. */
+tc_status tc_radon_static(tc_plan *plan, const float *volume, int n_slices, float *sinogram, void *cuda_stream);
+
 /* Stage hooks for the per-stage unit tests: ONE complex plane through ONE stage of the NUFFT, HOST arrays in natural order
  * (complex = interleaved float pairs).  fine_grid: F1 + F2 of eq. (8) read backwards: slices re, im (im nullable) ->
  * Ghat[k_y][k_x], G x G, G = 2 n, FFT order, of the plane re + i im (deapodised, zero-padded, 2-D FFT); gather: F3, eq. (7) reversed

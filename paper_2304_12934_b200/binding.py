@@ -53,6 +53,7 @@ lib.tc_plan_create.argtypes = [ctypes.POINTER(tc_geom), _ci, ctypes.POINTER(_vp)
 lib.tc_plan_destroy.argtypes = [_vp]
 lib.tc_radon.argtypes = [_vp, _vp, _ci, _vp, _vp]
 lib.tc_backproject.argtypes = [_vp, _vp, _ci, _vp, _vp]
+lib.tc_radon_static.argtypes = [_vp, _vp, _ci, _vp, _vp]
 lib.tc_fbp.argtypes = [_vp, _vp, _ci, _ci, _vp, _vp]
 lib.tc_mbir.argtypes = [_vp, _vp, _ci, ctypes.POINTER(tc_prior), _ci, _vp, ctypes.POINTER(tc_iter_log), _vp]
 lib.tc_mbir_sharded.argtypes = [_vp, _vp, _ci, ctypes.POINTER(tc_prior), _ci, _vp, ctypes.POINTER(tc_iter_log), ctypes.POINTER(tc_comm), _vp]
@@ -137,6 +138,11 @@ class Plan:
         assert tuple(volume.shape) == (S, self.n, self.n)
         out = _like(volume, (S, self.n_angles, self.n_det)) if out is None else out
         _check(lib.tc_radon(self._h, _ptr(volume), S, _ptr(out), _stream(volume)))
+        return out
+
+    def radon_static(self, volume, out):
+        """tc_radon_static: device tensors only, `out` preallocated by the caller (nothing is allocated on the way)."""
+        _check(lib.tc_radon_static(self._h, _ptr(volume), int(volume.shape[0]), _ptr(out), _stream(volume)))
         return out
 
     def backproject(self, sinogram, out=None):

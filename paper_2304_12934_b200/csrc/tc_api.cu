@@ -48,6 +48,7 @@ struct tc_plan {
     long long n_taps = 0;
     unsigned *pair_offs = nullptr; int *pair_idx = nullptr; void *pair_w = nullptr;      // lists of the cell runs
     int *gt_tiles = nullptr; unsigned *gt_start = nullptr; int4 *gt_samples = nullptr;   // tile-binned gather tables
+    float2 *static_scratch = nullptr;   // device address of g_static_scratch on the plan's device (tc_radon_static); null if the lookup failed
     bool gather_tiles = true;     // F3 as k_fwd_gather_tiles + k_fwd_radial (default) or as the fused ray-by-ray k_fwd_gather (TC_GATHER=ray)
     // scratch
     int ng_alloc = 0;
@@ -93,6 +94,34 @@ static void prof_stage(tc_plan *p, int stage, cudaStream_t st, bool begin) {
 static const char *const STAGE_NAMES[TC_N_STAGES] = {"F1 fwd_rows", "F2 fwd_cols", "F3 fwd_gather", "B1 adj_radial", "B2 adj_spread", "B3 adj_cols", "B3+B4 adj_rows", "F4 fwd_radial"};
 struct NvtxRange { explicit NvtxRange(const char *name) { nvtxRangePushA(name); } ~NvtxRange() { nvtxRangePop(); } };
 #define STAGE(id, call) do { NvtxRange nv_(STAGE_NAMES[id]); prof_stage(p, id, st, true); call; prof_stage(p, id, st, false); } while (0)
+
+// ---- scratch of the allocation-free forward projection (tc_radon_static) --------------------------------------------------------
+// Callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it) get ONE entry point whose
+// FFT scratch is this file-scope array instead of the plan's lazily allocated buffers: fine grid, forward half-plane and polar
+// coefficients of ONE group of 8 slices, for n <= 256 and n_angles * n_det <= 131072 (16 MiB, held by every GPU that loads the
+// library until exit).  In host code the name `g_static_scratch` is a host-side stand-in, not a device address: the address is
+// taken with cudaGetSymbolAddress here, at set-up, once per device, with that device current, and handed to the kernels as a pointer.
+constexpr int TC_STATIC_MAX_N = 256;
+constexpr size_t TC_STATIC_MAX_SAMPLES = 131072;                                          // n_angles * n_det
+constexpr size_t TC_STATIC_GRID = (size_t)(2 * TC_STATIC_MAX_N) * (2 * TC_STATIC_MAX_N) * P;   // float2 elements: 8 MiB
+constexpr size_t TC_STATIC_ROW = (size_t)TC_STATIC_MAX_N * (2 * TC_STATIC_MAX_N) * P;          // 4 MiB
+constexpr size_t TC_STATIC_CPOL = TC_STATIC_MAX_SAMPLES * P;                                  // 4 MiB
+static __device__ __align__(256) float2 g_static_scratch[TC_STATIC_GRID + TC_STATIC_ROW + TC_STATIC_CPOL];
+
+static float2 *static_scratch_address() {
+    constexpr int MAX_DEV = 64;
+    static float2 *addr[MAX_DEV] = {nullptr};
+    static bool tried[MAX_DEV] = {false};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEV) { cudaGetLastError(); return nullptr; }
+    if (!tried[dev]) {
+        tried[dev] = true;
+        void *q = nullptr;
+        if (cudaGetSymbolAddress(&q, g_static_scratch) == cudaSuccess) addr[dev] = static_cast<float2 *>(q);
+        else cudaGetLastError();                                     // tc_radon_static then fails with a clear error; nothing else uses it
+    }
+    return addr[dev];
+}
 
 // ---- host-side mathematics of the plan (float64) ---------------------------------------------------
 static double bessel_i0(double x) {          // I0(x) = sum_k (x^2/4)^k / (k!)^2
@@ -406,6 +435,7 @@ extern "C" tc_status tc_plan_create(const tc_geom *gm, int max_slab_slices, tc_p
         const char *env = std::getenv("TC_GATHER");
         p->gather_tiles = !(env && std::string(env) == "ray") || W != KB_W;      // the ray-by-ray kernel is built for W = 6 only
     }
+    p->static_scratch = static_scratch_address();     // set-up: tc_radon_static itself makes no symbol lookup
     *out = p;
     return TC_OK;
 }
@@ -569,3 +599,32 @@ struct CallMem {
 
 #include "tc_ops.cuh"
 #include "tc_mbir_streamed.cuh"
+
+// ---- allocation-free forward projection --------------------------------------------------------------------------------------------
+// tc_radon for DEVICE pointers with the FFT scratch in g_static_scratch (above): no cudaMalloc, cudaFree or allocating library
+// routine, whatever the plan has or has not allocated so far.  Slices go through in groups of 8, one after the other on `stream`.
+// Nothing in the scratch has to start at zero (the half-plane and the polar coefficients are fully rewritten for every group, and
+// the fine-grid cells the column kernel does not write are never used by the gather), so nothing is cleared; the array keeps the
+// last call's contents.  EVERY call on a device shares the array: calls that overlap on the GPU (two streams, two plans, two host
+// threads) race.
+extern "C" tc_status tc_radon_static(tc_plan *p, const float *volume, int S, float *sinogram, void *stream) {
+    if (!p || !volume || !sinogram) return fail(TC_EINVAL, "null argument");
+    if (S <= 0) return fail(TC_EINVAL, "n_slices must be positive");
+    const DevPlan &d = p->d;
+    if (d.n > TC_STATIC_MAX_N || (size_t)d.na * d.nd > TC_STATIC_MAX_SAMPLES)
+        return fail(TC_EUNSUPPORTED, "tc_radon_static: the static scratch holds n <= 256 and n_angles * n_det <= 131072 (this plan: n = " +
+                                         std::to_string(d.n) + ", n_angles * n_det = " + std::to_string((size_t)d.na * d.nd) + "); use tc_radon");
+    if (!p->static_scratch) return fail(TC_ECUDA, "tc_radon_static: cudaGetSymbolAddress of the static scratch failed at plan creation");
+    if (!is_device_ptr(volume) || !is_device_ptr(sinogram)) return fail(TC_EINVAL, "tc_radon_static: device pointers only");
+    float2 *grid = p->static_scratch, *rowbuf = grid + TC_STATIC_GRID, *cpol = rowbuf + TC_STATIC_ROW;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t vps = (size_t)d.n * d.n, sps = (size_t)d.na * d.nd;
+    for (int s0 = 0; s0 < S; s0 += 8) {
+        const int ns = std::min(8, S - s0);
+        launch_fwd_rows(d, volume + (size_t)s0 * vps, ns, 1, rowbuf, st);
+        launch_fwd_cols(d, rowbuf, 1, grid, st);
+        launch_fwd_gather_tiles(d, grid, 1, cpol, st);
+        launch_fwd_radial(d, cpol, ns, 1, sinogram + (size_t)s0 * sps, st);
+    }
+    return check_launch();
+}
