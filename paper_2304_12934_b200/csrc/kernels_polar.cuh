@@ -333,11 +333,15 @@ __global__ void __launch_bounds__(256) k_adj_spread_heavy(DevPlan d, const unsig
 // axis share most of their samples (two cells: 42 instead of 72 per full footprint; four: 54 instead of 144), so a lane pair now
 // owns a run of SP_NC cells (ix0 .. ix0 + NC - 1, ix0 a multiple of NC) and walks the union of their lists, (sample, one weight per
 // cell): the same FMAs plus those with a zero weight, which leave the sum unchanged: the result is bit-identical to the per-cell
-// form.  Lists are plan-time data as before; the first SP_NR entries stay in registers across the groups of the slab.
-constexpr int SP_NR = SP_NC == 2 ? 8 : 6;                 // list entries kept in registers
+// form.  Lists are plan-time data as before; the first SP_NR entries stay in registers across the groups of the slab (the rest is
+// re-read from L1 / L2 per block of groups).
+#ifndef SP_NR_
+#define SP_NR_ (SP_NC == 2 ? 4 : 6)      // 4 entries + four CTAs per SM (64 registers) measured 2.71 ms against 2.79 ms for 8 entries + three CTAs
+#endif
+constexpr int SP_NR = SP_NR_;                             // list entries kept in registers
 constexpr int SP_RUNS = 256 / SP_NC;                      // runs per 32 x 8 tile
 #ifndef SP_LB
-#define SP_LB (SP_NC == 2 ? 3 : 4)                        // CTAs per SM the main kernel is compiled for
+#define SP_LB 4                        // CTAs per SM the main kernel is compiled for
 #endif
 struct SpW { float w[SP_NC]; };
 
