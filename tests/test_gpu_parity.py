@@ -439,6 +439,35 @@ def test_tma_line_kernels_ragged_groups_and_unaligned_input(tc):
     assert rel_l2(s2, s) < 1e-6 and rel_l2(b2, b) < 1e-6
 
 
+def test_two_plans_alive_and_interleaved(tc):
+    # Plan state is per plan (window polynomial, tables, scratch) and the tensor-map caches of the TMA kernels are keyed by buffer:
+    # two plans with different window widths and geometries, used alternately, each against the oracle; then a plan is destroyed and a
+    # new one of another size takes its place (its scratch may land where the old one's was).
+    from paper_2304_12934_b200 import inputs
+    from oracle import nufft
+    rng = np.random.default_rng(91)
+    Na = 12
+    ang = inputs.angles_uniform(Na); a64 = ang.astype(np.float64)
+    pa = tc.Plan(1024, 1024, ang, 514.5, kb_width=6)                # TMA line kernels
+    pb = tc.Plan(128, 96, ang, 47.0, kb_width=8)                    # plain kernels, radix-3 detector, other window
+    va = inputs.volume_porous(3, 1024, 92); vb = rng.random((9, 128, 128)).astype(np.float32)
+    ya = rng.standard_normal((3, Na, 1024)).astype(np.float32); yb = rng.standard_normal((9, Na, 96)).astype(np.float32)
+    sa0 = _np(pa.radon(_cuda(va))); sb0 = _np(pb.radon(_cuda(vb)))
+    ba0 = _np(pa.backproject(_cuda(ya))); bb0 = _np(pb.backproject(_cuda(yb)))
+    sa1 = _np(pa.radon(_cuda(va))); bb1 = _np(pb.backproject(_cuda(yb)))
+    assert np.array_equal(sa0, sa1) and np.array_equal(bb0, bb1)                      # deterministic, no cross-talk
+    assert rel_l2(sa0[1], nufft.radon_nufft(va[1], a64, 1024, 514.5)) < TOL_NUFFT
+    assert rel_l2(ba0[2], nufft.backproject_nufft(ya[2], a64, 1024, 514.5)) < TOL_NUFFT
+    assert rel_l2(sb0, nufft.radon_nufft(vb, a64, 96, 47.0, W=8)) < TOL_NUFFT
+    assert rel_l2(bb0, nufft.backproject_nufft(yb, a64, 128, 47.0, W=8)) < TOL_NUFFT
+    pa.close()
+    pc = tc.Plan(1024, 1024, ang, 500.0, kb_width=4)                # same size class, new plan, other centre and window
+    sc = _np(pc.radon(_cuda(va[:1])))
+    assert rel_l2(sc[0], nufft.radon_nufft(va[0], a64, 1024, 500.0, W=4)) < TOL_NUFFT
+    assert np.array_equal(_np(pb.radon(_cuda(vb))), sb0)
+    pb.close(); pc.close()
+
+
 def test_second_workload_shape_2448_bins(tc):
     # the shape of the paper's third data set (202 projections x 2448 columns, Table 1) on a 2560^2 image:
     # n_det = 2448 = 2^4 3^2 17 runs the radix-3 and radix-17 passes of the radial FFT, n_det != n puts 2.09 fine-grid cells between
