@@ -354,7 +354,10 @@ def main():
              "fwd_pairs_per_s": S * Na / (sum(per[k][0] * per[k][1] for k in per if k.startswith("fwd")) / nprof * 1e-3),
              "adj_pairs_per_s": S * Na / (sum(per[k][0] * per[k][1] for k in per if k.startswith("adj")) / nprof * 1e-3),
              "step_model_bytes": model_bytes, "step_frac_of_hbm_roofline": model_bytes / (secs / args.steps) / 1e9 / peak,
-             "step_frac_of_nominal_8TBs": model_bytes / (secs / args.steps) / 8e12}
+             "step_frac_of_nominal_8TBs": model_bytes / (secs / args.steps) / 8e12,
+             # also against the compulsory bytes (inputs + outputs only, 8 N^2 + 8 Na Nd per slice)
+             "step_compulsory_bytes": (8 * N * N + 8 * Na * Nd) * S,
+             "step_frac_of_compulsory_roofline": (8 * N * N + 8 * Na * Nd) * S / (secs / args.steps) / 1e9 / peak}
 
     # ---- e2e: host buffers through the C ABI (slab scheduler) ----
     e2e = None
