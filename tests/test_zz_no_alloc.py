@@ -26,13 +26,18 @@ def test_radon_static_matches_tc_radon_on_two_calls_in_a_row():
     vol1 = torch.from_numpy(inputs.volume_cfg2()).cuda()
     plan1 = tc.Plan(c["N"], c["Nd"], ang1, c["centre"])
     out1 = torch.empty((c["S"], c["Na"], c["Nd"]), dtype=torch.float32, device="cuda")
-    torch.cuda.synchronize()
-    free0 = torch.cuda.mem_get_info()[0]
     plan1.radon_static(vol1, out1)                                   # before any other call on this plan: its own scratch does not exist yet
+    out1c = torch.empty_like(out1)
+    ref_buf = torch.empty_like(out1)
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]                             # after the first call, so that one-time loading of kernel code is not counted
+    plan1.radon_static(vol1, out1c)
     torch.cuda.synchronize()
     assert torch.cuda.mem_get_info()[0] == free0, "tc_radon_static allocated device memory"
-    ref1 = plan1.radon(vol1)                                         # the existing path (allocates the plan's scratch)
+    assert torch.equal(out1c, out1)
+    ref1 = plan1.radon(vol1, out=ref_buf)                            # the existing path: only now does the plan allocate its scratch
     torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] < free0, "the plan's own scratch existed already: the check above proved nothing"
     assert rel_l2(out1.cpu().numpy(), ref1.cpu().numpy()) <= TOL_SAME_PATH
     assert rel_l2(out1[3].cpu().numpy(), nufft.radon_nufft(vol1[3].cpu().numpy(), ang1.astype(np.float64), c["Nd"], c["centre"])) < TOL_NUFFT
 
