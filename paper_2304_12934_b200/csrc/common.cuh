@@ -117,8 +117,9 @@ void launch_update(const float *x, const float *xm, float beta, const float *atr
 // z = y - alpha g (projected on z >= 0 if nonneg), y as above     (candidate of the majorise-minimise step)
 void launch_step(const float *x, const float *xm, float beta, const float *g, float alpha, int nonneg, float *z, size_t n, cudaStream_t st);
 // Az = Ay - alpha Ag, Ay = A0 + beta (A0 - A1) (A1 == nullptr: Ay = A0; Ag == nullptr: Az = Ay);  acc[0] += 1/2 ||Az - b||^2   (M4 data term)
+// rnext (nullable; may alias Ag): the next iteration's residual if the candidate is accepted, Az + beta_next (Az - A0) - b (A0 must be A x)
 void launch_candidate_sino(const float *A0, const float *A1, const float *Ag, const float *b, float beta, float alpha, float *Az, double *acc,
-                           size_t n, cudaStream_t st);
+                           size_t n, cudaStream_t st, float *rnext = nullptr, float beta_next = 0.f);
 // acc[1] += H(z) over unordered neighbour pairs (M4 prior term); grad (nullable) = grad H(z)
 // pairs are owned by their lower slice; only owners among the first S_own slices are summed (S_own < 0: all)
 void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, int n, cudaStream_t st, int S_own = -1);

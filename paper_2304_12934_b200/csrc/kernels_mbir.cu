@@ -57,17 +57,22 @@ __global__ void k_residual(const float *__restrict__ Ax, const float *__restrict
         r[i] = fmaf(beta, a - Axm[i], a) - b[i];
     }
 }
-// Az = A y - alpha A g (A y from A0, A1 as above; A1 == nullptr: A0 is A y itself; Ag == nullptr: Az = A y) and the data term.
+// Az = A y - alpha A g (A y from A0, A1 as above; A1 == nullptr: A0 is A y itself; Ag == nullptr: Az = A y) and the data term;
+// optionally (rnext, only meaningful when A0 is A x) the next iteration's residual Az + beta_next (Az - A0) - b.
 // No __restrict__: Az may alias any input (each thread reads its own elements before it writes them).
 __global__ void k_candidate_sino(const float *A0, const float *A1, const float *Ag, const float *b, float beta, float alpha,
-                                 float *Az, double *partials, size_t n) {
+                                 float *Az, double *partials, size_t n, float *rnext, float beta_next) {
     double s = 0.0;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         const float a = A0[i];
         const float ay = A1 ? fmaf(beta, a - A1[i], a) : a;
         const float az = Ag ? fmaf(-alpha, Ag[i], ay) : ay;
+        const float bi = b[i];
         Az[i] = az;
-        const double e = (double)az - (double)b[i];
+        // the residual of the NEXT iteration if this candidate is accepted (then A x = A z, A x- = A0): the expression of k_residual,
+        // on values this thread holds anyway; rnext may alias Ag (read above)
+        if (rnext) rnext[i] = fmaf(beta_next, az - a, az) - bi;
+        const double e = (double)az - (double)bi;
         s += e * e;
     }
     block_reduce_to(s, partials);
@@ -409,9 +414,9 @@ void launch_step(const float *x, const float *xm, float beta, const float *g, fl
     k_step<<<ew_blocks(n), 256, 0, st>>>(x, xm, beta, g, alpha, nonneg, z, n); TC_COUNT_LAUNCH();
 }
 void launch_candidate_sino(const float *A0, const float *A1, const float *Ag, const float *b, float beta, float alpha, float *Az, double *acc,
-                           size_t n, cudaStream_t st) {
+                           size_t n, cudaStream_t st, float *rnext, float beta_next) {
     // second half of the partial-sum area: this reduction may run beside the prior's (launch_prior) on another stream
-    k_candidate_sino<<<RED_BLOCKS, RED_THREADS, 0, st>>>(A0, A1, Ag, b, beta, alpha, Az, acc + 16 + 2048, n); TC_COUNT_LAUNCH();
+    k_candidate_sino<<<RED_BLOCKS, RED_THREADS, 0, st>>>(A0, A1, Ag, b, beta, alpha, Az, acc + 16 + 2048, n, rnext, beta_next); TC_COUNT_LAUNCH();
     final_reduce(acc, 0, 0.5, st, 1);
 }
 void launch_prior(const float *z, PriorDev pr, float *grad, double *acc, int S, int n, cudaStream_t st, int S_own) {

@@ -379,6 +379,7 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
     auto slabbed = [&](slab_op op, const float *in, size_t ips, float *out, size_t ops) {
         for (int s0 = 0; s0 < S; s0 += slab) op(p, in + (size_t)s0 * ips, std::min(slab, S - s0), out + (size_t)s0 * ops, st);
     };
+    bool r_ready = false;                                                 // r holds the coming iteration's residual (written by k_candidate_sino)
     for (int it = 0; it < iters; ++it) {
         NvtxRange nv_it("tc_mbir iteration");
         const double tp = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));
@@ -387,7 +388,8 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
             slabbed(forward_slab, x, vps, Ax, sps);
             slabbed(forward_slab, xm, vps, Axm, sps);
         }
-        launch_residual(Ax, Axm, b, beta, r, ns, st);                     // M1 (sinogram part): r = A y - b
+        if (it > 0 && it % AX_REFRESH == 0) r_ready = false;
+        if (!r_ready) launch_residual(Ax, Axm, b, beta, r, ns, st);       // M1 (sinogram part): r = A y - b (else: left there by the last candidate kernel)
         slabbed(adjoint_slab, r, sps, gv, vps);                           // A^T (A y - b)
         CU(cudaMemsetAsync(p->acc, 0, 16 * sizeof(double), st));
         float alpha = invL;
@@ -418,7 +420,10 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
         } else {
             if (!pr->mm_step) slabbed(forward_slab, gv, vps, r, sps);     // A g
             if (sd != st) { CU(cudaEventRecord(p->ev_aux[0], st)); CU(cudaStreamWaitEvent(sd, p->ev_aux[0], 0)); }
-            launch_candidate_sino(Ax, Axm, r, b, beta, alpha, Az, p->acc, ns, sd);            // M4: Az = A y - alpha A g
+            // M4: Az = A y - alpha A g; the same pass leaves, in place of A g, the residual of the next iteration for the case that this
+            // candidate is accepted without a restart (the momentum of that iteration is known now: t becomes tp)
+            const double tp2 = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * tp * tp));
+            launch_candidate_sino(Ax, Axm, r, b, beta, alpha, Az, p->acc, ns, sd, r, (float)((tp - 1.0) / tp2));
         }
         if (sd != st) CU(cudaEventRecord(p->ev_aux[1], sd));
         if (comm) {                                                       // the candidate's boundary slices go to the neighbours' halos
@@ -445,7 +450,9 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
             x = xe + co; xm = xme + co; z = ze + co;
             float *oa = Axm; Axm = Ax; Ax = Az; Az = oa;
             Fx = Fz; t = restarted ? 1.0 : tp;
+            r_ready = !restarted && !pd.nonneg;                           // r already holds A y - b of the next iteration
         } else {
+            r_ready = false;
             t = 1.0;                                                      // restart: the next step is a plain gradient step from x (beta = 0)
         }
         if (log) { log[it].F = Fx; log[it].data = h[0]; log[it].prior = h[1]; log[it].margin = margin; log[it].beta = beta; log[it].accepted = accept ? 1 : 0;
