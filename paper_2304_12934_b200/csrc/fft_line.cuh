@@ -53,8 +53,8 @@ template <int PL_> struct RCfgT {
 };
 
 // Plane-major last pass: thread = (plane, slot) instead of (slot, plane), so a warp's stores are 32 consecutive outputs of ONE
-// plane (a full 128-byte line per float slice) -- for kernels whose output is the float volume, at the price of 4-way bank
-// conflicts on that pass's shared-memory reads.
+// plane (a full 128-byte line per float slice) -- for kernels whose output is the float volume.  In the [cell][plane] layout that
+// pass's shared-memory reads have 4-way bank conflicts; the grouped kernels stage the data plane-major first (line_mid_pm).
 template <class Base> struct PlaneMajorLast : Base { static constexpr bool PM_LAST = true; };
 
 // Grouped form: a CTA holds several independent groups of GT threads (GT = SLOTS * PL), each transforming its own line in its own
@@ -250,6 +250,65 @@ __device__ __forceinline__ void line_last(const LineCtx &c, const Cfg &cfg, PRE 
     }
 }
 
+// Plane-major staging for the plane-major last pass (PM_LAST): the last in-place pass leaves its results as [plane][cell] (plane
+// stride n + 8 cells, no padding cells) instead of [cell][plane], so that the last pass -- a warp = 32 consecutive tasks of ONE
+// plane -- reads consecutive 8-byte words (two wavefronts per instruction) instead of every fourth (eight).  The layout change is not
+// in place, so the pass reads, meets the group's barrier, then writes: one task per thread (n / R == SLOTS).
+template <class Cfg> __device__ __forceinline__ constexpr int pm_stride() { return Cfg::n() + 8; }
+template <int R, bool INV, class Cfg>
+__device__ __forceinline__ void line_mid_pm(const LineCtx &c, const Cfg &cfg, int s) {
+    constexpr int n = Cfg::n(), R1 = Cfg::radix(0);
+    static_assert(n / R == Cfg::SLOTS, "one task per thread");
+    const int ni = n / s, sub = ni / R;
+    const int T = c.slot;
+    const bool on = T < n / R;
+    float2 v[R];
+    int c0 = 0;
+    if (on) {
+        const int k1 = T % R1, rest = T / R1;
+        const int outer = rest / sub, bi = rest - outer * sub;
+        c0 = R1 * (outer * ni + bi) + k1;
+#pragma unroll
+        for (int j = 0; j < R; ++j) v[j] = c.sm[pcell(c0 + j * R1 * sub) * Cfg::PL + c.pl];
+        Bfly<R, INV>::run(v);
+        twiddle_mul<R, INV>(c.tw, bi * s * cfg.tws(), v, n * cfg.tws());
+    }
+    line_sync<Cfg>();                                   // every task has its inputs: the buffer may change layout
+    if (on) {
+        float2 *o = c.sm + c.pl * pm_stride<Cfg>() + c0;
+#pragma unroll
+        for (int j = 0; j < R; ++j) o[j * R1 * sub] = v[j];
+    }
+    line_sync<Cfg>();
+}
+template <int R, bool INV, class Cfg, class PRE, class ST>
+__device__ __forceinline__ void line_last_pm(const LineCtx &c, const Cfg &cfg, PRE pre, ST st) {
+    constexpr int n = Cfg::n(), R1 = Cfg::radix(0), ntask = n / R;
+    const int my_pl = line_tid<Cfg>() / Cfg::SLOTS, my_slot = line_tid<Cfg>() % Cfg::SLOTS;
+#pragma unroll 1
+    for (int T = my_slot; T < ntask; T += Cfg::SLOTS) {
+        const int k1 = T % R1;
+        int rem = T / R1, mult = n / R1, B0 = 0;
+#pragma unroll
+        for (int i = 1; i + 1 < cfg.npass(); ++i) {
+            const int Ri = cfg.radix(i);
+            mult /= Ri;
+            const int q = rem / Ri;
+            B0 += (rem - q * Ri) * mult;
+            rem = q;
+        }
+        const float2 *p0 = c.sm + my_pl * pm_stride<Cfg>() + R1 * B0 + k1;
+        float2 v[R], old[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) old[k] = pre(T + ntask * k, R % 2 == 0 ? k < R / 2 : 2 * (T + ntask * k) < n);
+#pragma unroll
+        for (int j = 0; j < R; ++j) v[j] = p0[j * R1];
+        Bfly<R, INV>::run(v);
+#pragma unroll
+        for (int k = 0; k < R; ++k) st(T + ntask * k, R % 2 == 0 ? k < R / 2 : 2 * (T + ntask * k) < n, v[k], old[k]);
+    }
+}
+
 template <class Cfg>
 __device__ __forceinline__ LineCtx line_ctx(float2 *sm, const float2 *tw) {
     LineCtx c;
@@ -264,10 +323,14 @@ template <bool INV, class Cfg, int I, int S_, class PRE, class ST>
 __device__ __forceinline__ void static_finish(const LineCtx &c, const Cfg &cfg, PRE pre, ST st) {
     constexpr int R = Cfg::radix(I);
     if constexpr (I + 1 < Cfg::NP) {
-        line_mid<R, INV>(c, cfg, S_);
+        if constexpr (I + 2 == Cfg::NP && Cfg::PM_LAST && Cfg::GROUP_THREADS != 0 && Cfg::n() / R == Cfg::SLOTS) line_mid_pm<R, INV>(c, cfg, S_);
+        else line_mid<R, INV>(c, cfg, S_);
         static_finish<INV, Cfg, I + 1, S_ * R>(c, cfg, pre, st);
     } else {
-        line_last<R, INV>(c, cfg, pre, st);
+        if constexpr (Cfg::PM_LAST && Cfg::GROUP_THREADS != 0 && I >= 2) {      // the grouped (TMA-fed) kernels only: the plain ones lose more on the extra barrier (2.48 -> 2.98 ms)
+            if constexpr (Cfg::n() / Cfg::radix(I - 1) == Cfg::SLOTS) line_last_pm<R, INV>(c, cfg, pre, st);
+            else line_last<R, INV>(c, cfg, pre, st);
+        } else line_last<R, INV>(c, cfg, pre, st);
     }
 }
 
