@@ -395,14 +395,14 @@ def main():
         pr = tc.prior_params(L=step_L(Na, N))
         plan.mbir(b, pr, 1); fence()
 
-        def t_mbir(its):                                           # min of 3: buffer allocation inside the call varies
-            best = 1e30
-            for _ in range(3):
-                t0 = time.perf_counter(); plan.mbir(b, pr, its); fence(); best = min(best, time.perf_counter() - t0)
-            return best
-        nit = int(min(40, max(8, 800.0 / (2.3 * ms_step))))        # enough iterations for ~0.8 s between the two timings (below AX_REFRESH = 50):
-        t2, t8 = t_mbir(2), t_mbir(2 + nit)                       # the calls' fixed costs (allocation of the state, ||b||^2, copy out) vary by a few ms
-        it_s = max_over_ranks((t8 - t2) / nit)
+        # every iteration ends with a stream synchronisation (the accept test), and the library logs the wall time between two of
+        # them (tc_iter_log.ms): the median over the iterations of one call, first iteration left out.  (Differences of whole-call
+        # times are useless here: allocation and release of the ~10 GB of state vary by milliseconds from call to call.)
+        nit = 24
+        _, logm = plan.mbir(b, pr, nit); fence()
+        _, logm = plan.mbir(b, pr, nit); fence()
+        it_s = max_over_ranks(float(np.median([l["ms"] for l in logm[1:]])) * 1e-3)
+        extra["mbir_iter_ms_min_max"] = [float(min(l["ms"] for l in logm[1:])), float(max(l["ms"] for l in logm[1:]))]
         extra["mbir_iter_ms"] = 1e3 * it_s
         extra["mbir_pairs_per_s"] = world * S * Na / it_s
         extra["mbir_model_bytes"] = (128 * N * N + 40 * Na * Nd) * S      # one MBIR iteration per slice
@@ -417,8 +417,7 @@ def main():
             pr3 = tc.prior_params(L=step_L(c3["Na"], c3["N"]))
             p3.mbir(b3, pr3, 2); fence()
             t0 = time.perf_counter(); x3, log3 = p3.mbir(b3, pr3, 50); fence(); t50 = time.perf_counter() - t0
-            t0 = time.perf_counter(); p3.mbir(b3, pr3, 10); fence(); t10 = time.perf_counter() - t0
-            it3 = (t50 - t10) / 40
+            it3 = float(np.median([l["ms"] for l in log3[1:]])) * 1e-3
             extra["cfg3_mbir_50it_s"] = t50
             extra["cfg3_mbir_iter_ms"] = 1e3 * it3
             extra["cfg3_mbir_pairs_per_s"] = c3["S"] * c3["Na"] / it3

@@ -63,8 +63,10 @@ typedef struct { float p, sigma, c, lambda, L; int nonneg, grad_restart, neighbo
 
 /* One record per MBIR iteration: F = objective of the kept iterate, data / prior = the two terms of
  * the CANDIDATE, margin = (F_prev - F_cand)/F_prev, dot = <g, z - x> (0 unless grad_restart), beta = momentum used,
- * accepted = 1/0, restarted = 1 if the gradient test reset the momentum, alpha = step length used (1/L unless mm_step). */
-typedef struct { double F, data, prior, margin, dot; float beta; int accepted, restarted; float alpha; } tc_iter_log;
+ * accepted = 1/0, restarted = 1 if the gradient test reset the momentum, alpha = step length used (1/L unless mm_step),
+ * ms = wall-clock milliseconds of this iteration (every iteration ends with a stream synchronisation for the accept test, so
+ * this is the GPU time of the iteration plus its launch overhead; bench.py's MBIR figure is the median of these). */
+typedef struct { double F, data, prior, margin, dot; float beta; int accepted, restarted; float alpha; float ms; } tc_iter_log;
 
 typedef struct tc_plan tc_plan;
 

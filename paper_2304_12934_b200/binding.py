@@ -30,7 +30,7 @@ class tc_prior(ctypes.Structure):
 class tc_iter_log(ctypes.Structure):
     _fields_ = [("F", ctypes.c_double), ("data", ctypes.c_double), ("prior", ctypes.c_double),
                 ("margin", ctypes.c_double), ("dot", ctypes.c_double), ("beta", ctypes.c_float), ("accepted", ctypes.c_int),
-                ("restarted", ctypes.c_int), ("alpha", ctypes.c_float)]
+                ("restarted", ctypes.c_int), ("alpha", ctypes.c_float), ("ms", ctypes.c_float)]
 
 
 class tc_sched_stats(ctypes.Structure):
@@ -165,7 +165,7 @@ class Plan:
         out = _like(sinogram, (S, self.n, self.n)) if out is None else out
         log = (tc_iter_log * max(iters, 1))()
         _check(lib.tc_mbir(self._h, _ptr(sinogram), S, ctypes.byref(prior), int(iters), _ptr(out), log, _stream(sinogram)))
-        recs = [dict(F=l.F, data=l.data, prior=l.prior, margin=l.margin, dot=l.dot, beta=l.beta, accepted=l.accepted, restarted=l.restarted, alpha=l.alpha)
+        recs = [dict(F=l.F, data=l.data, prior=l.prior, margin=l.margin, dot=l.dot, beta=l.beta, accepted=l.accepted, restarted=l.restarted, alpha=l.alpha, ms=l.ms)
                 for l in log[:iters]]
         return out, recs
 
@@ -198,7 +198,7 @@ class Plan:
         if errs:
             raise errs[0]
         _check(st)
-        recs = [dict(F=l.F, data=l.data, prior=l.prior, margin=l.margin, dot=l.dot, beta=l.beta, accepted=l.accepted, restarted=l.restarted, alpha=l.alpha)
+        recs = [dict(F=l.F, data=l.data, prior=l.prior, margin=l.margin, dot=l.dot, beta=l.beta, accepted=l.accepted, restarted=l.restarted, alpha=l.alpha, ms=l.ms)
                 for l in log[:iters]]
         return out, recs
 

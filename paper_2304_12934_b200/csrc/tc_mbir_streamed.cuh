@@ -72,6 +72,7 @@ static tc_status mbir_streamed(tc_plan *p, const float *hb, int S, const tc_prio
     double Fx = 0.5 * h[2], t = 1.0;
     auto t_begin = std::chrono::steady_clock::now();
     stt.setup_s = std::chrono::duration<double>(t_begin - t_setup).count();
+    auto t_iter = std::chrono::steady_clock::now();
     for (int it = 0; it < iters; ++it) {
         const double tp = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));
         const float beta = (float)((t - 1.0) / tp);
@@ -146,7 +147,8 @@ static tc_status mbir_streamed(tc_plan *p, const float *hb, int S, const tc_prio
         if (accept) { std::swap(U, V); Fx = Fz; t = restarted ? 1.0 : tp; }                       // x <- z, x- <- x: the two volumes swap roles
         else t = 1.0;                                                                              // V holds a dead candidate; the next step (beta = 0) does not read it
         if (log) { log[it].F = Fx; log[it].data = h[0]; log[it].prior = h[1]; log[it].margin = margin; log[it].beta = beta; log[it].accepted = accept ? 1 : 0;
-                   log[it].dot = pr->grad_restart ? h[3] : 0.0; log[it].restarted = restarted ? 1 : 0; log[it].alpha = invL; }
+                   log[it].dot = pr->grad_restart ? h[3] : 0.0; log[it].restarted = restarted ? 1 : 0; log[it].alpha = invL;
+                   const auto t_now = std::chrono::steady_clock::now(); log[it].ms = (float)std::chrono::duration<double, std::milli>(t_now - t_iter).count(); t_iter = t_now; }
     }
     auto t_end = std::chrono::steady_clock::now();
     stt.wall_s = std::chrono::duration<double>(t_end - t_begin).count();                          // the iterations

@@ -380,6 +380,7 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
         for (int s0 = 0; s0 < S; s0 += slab) op(p, in + (size_t)s0 * ips, std::min(slab, S - s0), out + (size_t)s0 * ops, st);
     };
     bool r_ready = false;                                                 // r holds the coming iteration's residual (written by k_candidate_sino)
+    auto t_iter = std::chrono::steady_clock::now();                       // tc_iter_log.ms: from one accept test's synchronisation to the next
     for (int it = 0; it < iters; ++it) {
         NvtxRange nv_it("tc_mbir iteration");
         const double tp = 0.5 * (1.0 + std::sqrt(1.0 + 4.0 * t * t));
@@ -456,7 +457,8 @@ static tc_status mbir_in_core(tc_plan *p, const float *sinogram, int S, const tc
             t = 1.0;                                                      // restart: the next step is a plain gradient step from x (beta = 0)
         }
         if (log) { log[it].F = Fx; log[it].data = h[0]; log[it].prior = h[1]; log[it].margin = margin; log[it].beta = beta; log[it].accepted = accept ? 1 : 0;
-                   log[it].dot = pr->grad_restart ? h[3] : 0.0; log[it].restarted = restarted ? 1 : 0; log[it].alpha = alpha; }
+                   log[it].dot = pr->grad_restart ? h[3] : 0.0; log[it].restarted = restarted ? 1 : 0; log[it].alpha = alpha;
+                   const auto t_now = std::chrono::steady_clock::now(); log[it].ms = (float)std::chrono::duration<double, std::milli>(t_now - t_iter).count(); t_iter = t_now; }
     }
     CU(cudaMemcpyAsync(volume, x, nv * sizeof(float), dev_v ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
